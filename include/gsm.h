@@ -1,0 +1,123 @@
+/* gsm.h - C ABI of the B200-native Generalized Source Method (GSM) hot path.
+ *
+ * Method: A.A. Shcherbakov, A.V. Tishchenko, "3D periodic dielectric composite homogenization based on the
+ * Generalized Source Method" (arxiv 1501.01752).  Citations "PAPER.md:<line>" refer to the text of that paper.
+ *
+ * What the library computes (Eq. 4, truncated to N1 x N2 x N3 harmonics):
+ *
+ *     E_{a,m} - sum_b G_{m;ab} sum_{m'} c_{m-m'} E_{b,m'} = a_a delta_{m,0}
+ *     G_{m;ab} = (k_b^2 delta_ab - k_{a,m} k_{b,m}) / (k_m.k_m - k_b^2),   k_m = k_bloch + (m1 K1, m2 K2, m3 K3),
+ *     K_a = 2 pi / Lambda_a,   k_b^2 = k0^2 eps_b,   c_d = (Delta eps / eps_b)_d  (Fourier coefficients of
+ *     (eps(r) - eps_b)/eps_b, plain Laurent rule).
+ *
+ * The operator y = x - G (T x) is applied with a zero-padded 3-D FFT convolution and the system is
+ * solved by full GMRES with modified Gram-Schmidt.  A scan over many (k_bloch, k0) points returns
+ * the 0-th order response used by the pole search of Eq. 6-10.
+ *
+ * Conventions
+ *   - All floating point is IEEE double; complex numbers are interleaved (re, im) doubles.
+ *   - Units: eps0 = mu0 = c = 1, relative permittivities; "omega" is passed as the vacuum wavenumber k0 = omega/c.
+ *   - Harmonic orders along axis a: m_a = i_a + mmin_a, i_a = 0..N_a-1, mmin_a = -(N_a-1)/2 for odd N_a and
+ *     -N_a/2 for even N_a.  Field layout: x[batch][3][N1][N2][N3], last index fastest.
+ *   - Coefficient layout (gsm_plan_coeffs): c[(2N1-1)][(2N2-1)][(2N3-1)], index d_a + N_a - 1.
+ *   - Pointer arguments are HOST pointers unless the name starts with d_ (DEVICE pointer, 16-byte aligned, on the
+ *     plan's device).  The caller owns every argument buffer; the plan owns all device scratch.
+ *   - Work is enqueued on the plan's CUDA stream.  gsm_apply returns without synchronising; every other call
+ *     returns after the host results it writes are valid.
+ *   - Errors are return codes (no exceptions, no abort, no CPU fallback).  Negative = failure, nothing valid
+ *     written; positive = warning, outputs written.  gsm_last_error gives a text for the last failure.
+ */
+#ifndef GSM_H_
+#define GSM_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gsm_plan gsm_plan; /* opaque: coefficient spectrum, FFT workspaces, Krylov pool on one device */
+
+typedef enum {
+    GSM_OK = 0,
+    GSM_NOT_CONVERGED = 1,     /* max_iters reached for at least one point; best iterate and history returned */
+    GSM_E_INVALID = -1,        /* bad argument (null pointer, size out of range, batch > max_batch, ...)       */
+    GSM_E_ALLOC = -2,          /* host or device allocation failed                                            */
+    GSM_E_CUDA = -3,           /* a CUDA runtime call or kernel launch failed                                 */
+    GSM_E_SINGULAR_BASIS = -4  /* min_m |k_m.k_m - k_b^2| / |k_b^2| < 1e-12: eps_b violates PAPER.md:52       */
+} gsm_status;
+
+enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2 };
+
+/* One analytic inclusion ("Fourier images of sphere and polyhedron can be combined").
+ * size = (R, -, -) for a sphere, semi-axes for an ellipsoid, full edge lengths for an axis-aligned box; same
+ * length unit as the periods.  The inclusion's permittivity replaces the background inside it; overlapping
+ * inclusions superpose their (eps_i - eps_bg) contrasts. */
+typedef struct {
+    int kind;
+    double center[3];
+    double size[3];
+    double eps_re, eps_im;
+} gsm_shape;
+
+/* Plan descriptor.  Exactly one of (n_shapes > 0, shapes) or (eps_grid_host != NULL) describes the cell.
+ * Voxel path: eps_grid_host[voxels[0]][voxels[1]][voxels[2]] complex, sample j at r_a = j_a Lambda_a / voxels[a];
+ * each voxels[a] must be a power of two with 2*orders[a]-1 <= voxels[a] <= 512 (the harmonics are taken from a
+ * device FFT of the grid), or 1 when orders[a] == 1. */
+typedef struct {
+    double period[3];            /* Lambda_1..3                 */
+    int orders[3];               /* N1..N3 harmonics kept per axis, 1 <= N <= 128                */
+    double eps_bg_re, eps_bg_im; /* background permittivity of the analytic path                               */
+    double eps_b_re, eps_b_im;   /* basis permittivity eps_b; must make every k_m^2 != k_b^2  */
+    int n_shapes;
+    const gsm_shape* shapes;
+    int voxels[3];
+    const double* eps_grid_host;
+    int max_iters;               /* GMRES basis size (unrestarted); default 64 if <= 0                         */
+    int max_batch;               /* (k, omega) points solved concurrently; default 1 if <= 0                   */
+    void* cuda_stream;           /* cudaStream_t to enqueue on; NULL = the legacy default stream               */
+} gsm_plan_desc;
+
+/* Build the plan on the current CUDA device: evaluate c_d (analytic closed forms or FFT of the voxel grid),
+ * embed it in the P1 x P2 x P3 circulant grid (P_a = smallest power of two >= 2 N_a - 1, 1 if N_a == 1), transform
+ * it once, allocate workspaces for max_batch concurrent solves.  *out is NULL on failure. */
+gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out);
+gsm_status gsm_plan_destroy(gsm_plan* plan);
+
+/* Test hook: copy the coefficients c_d the plan was built from (device result) to host_out,
+ * (2N1-1)(2N2-1)(2N3-1) complex numbers in the layout stated above. */
+gsm_status gsm_plan_coeffs(const gsm_plan* plan, double* host_out);
+
+/* FFT grid sizes P1..P3 chosen by the plan, device bytes held, and the number of kernel launches enqueued so far. */
+gsm_status gsm_plan_info(const gsm_plan* plan, int fft_grid[3], long long* device_bytes, long long* launches);
+
+/* Operator apply, Eq. 4 left-hand side: y[b] = x[b] - G(k_bloch[b], k0[b]) (T x[b]), b < batch.
+ * k_bloch[batch][3], k0[batch] are host arrays (copied before return).  d_x, d_y: device, [batch][3][N1][N2][N3]
+ * complex; they must not overlap.  1 <= batch <= max_batch.  Asynchronous on the plan's stream. */
+gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch, const double* k0, const void* d_x, void* d_y);
+
+/* One solve of Eq. 4 with right-hand side a delta_{m,0} by full GMRES from x0 = 0, stopping when
+ * the residual estimate |g_{j+1}| / ||b|| <= tol.  pol = complex amplitude a (3 complex).
+ * d_E_out: device, [3][N1][N2][N3] complex.  resid_hist_host (may be NULL): first min(n_iters, hist_cap) residual
+ * estimates.  n_iters: iterations used.  true_rel_resid: ||b - A E|| / ||b|| recomputed with one more apply. */
+gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double k0, const double pol[6], double tol,
+                     void* d_E_out, double* resid_hist_host, int hist_cap, int* n_iters, double* true_rel_resid);
+
+/* Scan: npts independent solves sharing the plan, run max_batch at a time in lock step.
+ * resp_host[npts][3] complex = E at m = 0; iters[npts]; resid[npts] = true relative residuals.
+ * d_E_out (may be NULL): device, [npts][3][N1][N2][N3] complex, all fields. */
+gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                    double tol, double* resp_host, int* iters, double* resid, void* d_E_out);
+
+/* Pole search, host side (Eq. 7-10, with xi in the numerator of Eq. 9 - DESIGN.md reading R11).
+ * kappa[npts] equidistant and increasing, xi[npts] complex, npts >= Np + Nd.  All npts - Nd sliding windows of
+ * Nd + 1 points are used (least squares).  eta[Np], zeta[Np] complex.  *best = index of the root with
+ * kappa_lo <= Re eta <= kappa_hi and the largest |zeta|, or -1. */
+gsm_status gsm_pole_search(int npts, const double* kappa, const double* xi, int Np, int Nd,
+                           double kappa_lo, double kappa_hi, double* eta, double* zeta, int* best);
+
+/* Text of the last failure on this plan (or of the last failed gsm_plan_create when plan == NULL). */
+const char* gsm_last_error(const gsm_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSM_H_ */
