@@ -1,0 +1,191 @@
+// apply.cu - the GSM operator y = x - G (T x) of Eq. 4 as three fused passes, complex fp64.
+//
+// (T x)_{c,m} = sum_m' c_{m-m'} x_{c,m'} is a 3-D Toeplitz product done by circulant embedding in a
+// P1 x P2 x P3 grid.  The zero padding is never stored and only the N^3 needed outputs are produced:
+//
+//   pass 1  z_forward   x[b][c][l][i3] --z-FFT (N3 valid in, P3 out)--> W[b][c][pos3][l]          l = i1*N2+i2
+//   pass 2  xy_conv     per (b,c,pos3): plane W[.][l] -> y-FFT -> x-FFT -> * Chat -> x-IFFT -> y-IFFT -> W (in place)
+//   pass 3  z_inverse   W[b][.][pos3][l] --z-IFFT (N3 valid out)--> F, then the Green dyadic of Eq. 4:
+//                       y_c = x_c - (k_b^2 F_c - k_c (k.F)) / (k.k - k_b^2)
+//
+// The intermediate W is only 2x (not 8x) the field: it is transformed along z alone.  Pass 2 keeps its plane in
+// shared memory pruned to N1 rows and expands along x one column batch at a time through a scratch tile, so a
+// 128 x 128 plane never has to exist.  FFT outputs stay in the digit-reversed "position" order of fft_device.cuh;
+// Chat is stored in the same order, [pos3][pos1][pos2], so the pass-2 read of Chat is contiguous along pos2.
+#include "gsm_internal.cuh"
+
+namespace gsm {
+
+static __device__ __forceinline__ void load_tw(cplx* dst, const cplx* __restrict__ src, int P) {
+    for (int i = threadIdx.x; i < P; i += blockDim.x) dst[i] = src[i];
+}
+
+// ---------------------------------------------------------------------------------------------------- pass 1
+__global__ void __launch_bounds__(256) z_forward_kernel(ApplyGeom g, const cplx* __restrict__ x, cplx* __restrict__ W,
+                                                        const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);
+    cplx* S = tw + g.ax[2].P;
+    const int P3 = g.ax[2].P, N3 = g.N3;
+    const int l0 = blockIdx.x * g.L;
+    const int nl = min(g.L, g.NL - l0);
+    load_tw(tw, g.tw[2], P3);
+    const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l0 * N3;
+    for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
+        const int l = i / N3, i3 = i - l * N3;
+        S[i3 * g.Lst + l] = xs[i];
+    }
+    __syncthreads();
+    fft_forward(g.ax[2], Lines{S, g.Lst, 1}, nl, tw, N3);
+    cplx* Wd = W + ((long)b * 3 + c) * P3 * g.NL + l0;
+    for (int i = threadIdx.x; i < nl * P3; i += blockDim.x) {
+        const int pos = i / nl, l = i - pos * nl;
+        Wd[(long)pos * g.NL + l] = S[pos * g.Lst + l];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------- pass 2
+__global__ void __launch_bounds__(256) xy_conv_kernel(ApplyGeom g, cplx* __restrict__ W, const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y, pos3 = blockIdx.x;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P1 = g.ax[0].P, P2 = g.ax[1].P, N1 = g.N1, N2 = g.N2;
+    cplx* tw1 = reinterpret_cast<cplx*>(smem_raw);
+    cplx* tw2 = tw1 + P1;
+    cplx* A = tw2 + P2;                // [P2][N1s]: A[k2 * N1s + i1]
+    cplx* B = A + (long)P2 * g.N1s;    // [P1][CBs]: B[k1 * CBs + col]
+    load_tw(tw1, g.tw[0], P1);
+    load_tw(tw2, g.tw[1], P2);
+    cplx* Wp = W + (((long)b * 3 + c) * g.ax[2].P + pos3) * g.NL;
+    for (int i = threadIdx.x; i < g.NL; i += blockDim.x) {
+        const int i1 = i / N2, i2 = i - i1 * N2;
+        A[i2 * g.N1s + i1] = Wp[i];
+    }
+    __syncthreads();
+    // y: N1 lines (index i1, contiguous), elements along k2 at stride N1s
+    fft_forward(g.ax[1], Lines{A, g.N1s, 1}, N1, tw2, N2);
+    // x: P2 lines (index k2, odd stride N1s), elements along i1 contiguous; CB columns at a time
+    const AxisPlan& ax = g.ax[0];
+    const cplx* chat = g.chat + (long)pos3 * P1 * P2;
+    for (int cb0 = 0; cb0 < P2; cb0 += g.CB) {
+        const int ncol = min(g.CB, P2 - cb0);
+        const Lines a{A + (long)cb0 * g.N1s, 1, g.N1s};
+        const Lines bb{B, g.CBs, 1};
+        if (ax.nst == 0) {
+            for (int i = threadIdx.x; i < ncol; i += blockDim.x)
+                a.p[i * a.ls] = cmul(a.p[i * a.ls], __ldg(chat + cb0 + i));
+            __syncthreads();
+            continue;
+        }
+        int Ls = P1;
+        for (int s = 0; s + 1 < ax.nst; ++s) {
+            dif_stage_rt(ax.radix[s], s == 0 ? a : bb, bb, ncol, P1, Ls, tw1, s == 0 ? N1 : P1);
+            Ls /= ax.radix[s];
+            __syncthreads();
+        }
+        const bool only = ax.nst == 1;
+        mid_stage_rt(ax.radix[ax.nst - 1], only ? a : bb, only ? a : bb, ncol, P1, chat + cb0, P2, 1, only ? N1 : P1,
+                     only ? N1 : P1);
+        __syncthreads();
+        for (int s = ax.nst - 2; s >= 0; --s) {
+            Ls *= ax.radix[s];
+            dit_stage_rt(ax.radix[s], bb, s == 0 ? a : bb, ncol, P1, Ls, tw1, s == 0 ? N1 : P1);
+            __syncthreads();
+        }
+    }
+    fft_inverse(g.ax[1], Lines{A, g.N1s, 1}, N1, tw2, N2);
+    for (int i = threadIdx.x; i < g.NL; i += blockDim.x) {
+        const int i1 = i / N2, i2 = i - i1 * N2;
+        Wp[i] = A[i2 * g.N1s + i1];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------- pass 3
+__global__ void __launch_bounds__(256) z_inverse_green_kernel(ApplyGeom g, const cplx* __restrict__ W,
+                                                              const cplx* __restrict__ x, cplx* __restrict__ y,
+                                                              const double* __restrict__ kvec,
+                                                              const double* __restrict__ k0s,
+                                                              const int* __restrict__ active) {
+    const int b = blockIdx.y;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P3 = g.ax[2].P, N3 = g.N3;
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);
+    cplx* S = tw + P3;                 // [P3][RS3]: S[pos * RS3 + c * nl + l]
+    const int l0 = blockIdx.x * g.L;
+    const int nl = min(g.L, g.NL - l0);
+    load_tw(tw, g.tw[2], P3);
+    for (int c = 0; c < 3; ++c) {
+        const cplx* Ws = W + ((long)b * 3 + c) * P3 * g.NL + l0;
+        for (int i = threadIdx.x; i < nl * P3; i += blockDim.x) {
+            const int pos = i / nl, l = i - pos * nl;
+            S[pos * g.RS3 + c * nl + l] = Ws[(long)pos * g.NL + l];
+        }
+    }
+    __syncthreads();
+    fft_inverse(g.ax[2], Lines{S, g.RS3, 1}, 3 * nl, tw, N3);
+    // Green dyadic: k_m = k_inc + m o K, k_b^2 = k0^2 eps_b, unconjugated k.k
+    const double kx0 = kvec[3 * b + 0], ky0 = kvec[3 * b + 1], kz0 = kvec[3 * b + 2], k0 = k0s[b];
+    const double kb2r = k0 * k0 * g.epsb_re, kb2i = k0 * k0 * g.epsb_im;
+    const long base = (long)b * 3 * g.n + (long)l0 * N3;
+    for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
+        const int l = i / N3, i3 = i - l * N3;
+        const int lg = l0 + l, i1 = lg / g.N2, i2 = lg - i1 * g.N2;
+        const double k1 = kx0 + (i1 + g.mmin[0]) * g.K[0];
+        const double k2 = ky0 + (i2 + g.mmin[1]) * g.K[1];
+        const double k3 = kz0 + (i3 + g.mmin[2]) * g.K[2];
+        const cplx F0 = S[i3 * g.RS3 + l], F1 = S[i3 * g.RS3 + nl + l], F2 = S[i3 * g.RS3 + 2 * nl + l];
+        const cplx s = make_double2(k1 * F0.x + k2 * F1.x + k3 * F2.x, k1 * F0.y + k2 * F1.y + k3 * F2.y);
+        const double dr = k1 * k1 + k2 * k2 + k3 * k3 - kb2r, di = -kb2i;
+        const double inv = 1.0 / (dr * dr + di * di);
+        const cplx rden = make_double2(dr * inv, -di * inv);   // 1 / (k.k - k_b^2)
+        const cplx kb2 = make_double2(kb2r, kb2i);
+        const cplx F[3] = {F0, F1, F2};
+        const double kk[3] = {k1, k2, k3};
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            cplx num = cmul(kb2, F[c]);
+            num.x -= kk[c] * s.x;
+            num.y -= kk[c] * s.y;
+            const cplx q = cmul(num, rden);
+            const cplx xv = x[base + c * g.n + i];
+            y[base + c * g.n + i] = make_double2(xv.x - q.x, xv.y - q.y);
+        }
+    }
+}
+
+static size_t smem_pass1(const ApplyGeom& g) { return sizeof(cplx) * ((size_t)g.ax[2].P + (size_t)g.ax[2].P * g.Lst); }
+static size_t smem_pass2(const ApplyGeom& g) {
+    return sizeof(cplx) * ((size_t)g.ax[0].P + g.ax[1].P + (size_t)g.ax[1].P * g.N1s + (size_t)g.ax[0].P * g.CBs);
+}
+static size_t smem_pass3(const ApplyGeom& g) { return sizeof(cplx) * ((size_t)g.ax[2].P + (size_t)g.ax[2].P * g.RS3); }
+
+size_t apply_smem_max(const ApplyGeom& g) {
+    size_t m = smem_pass1(g);
+    if (smem_pass2(g) > m) m = smem_pass2(g);
+    if (smem_pass3(g) > m) m = smem_pass3(g);
+    return m;
+}
+
+cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
+                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, long long* launches) {
+    const int nlt = (g.NL + g.L - 1) / g.L;
+    z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active);
+    xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active);
+    z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active);
+    if (launches) *launches += 3;
+    return cudaGetLastError();
+}
+
+}  // namespace gsm
+
+namespace gsm {
+cudaError_t apply_init_attributes() {
+    cudaError_t e = cudaFuncSetAttribute(z_forward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(xy_conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    return e;
+}
+}  // namespace gsm

@@ -1,0 +1,460 @@
+// gsm_api.cu - the C ABI of include/gsm.h: plan construction, operator apply, batched GMRES solve and scan.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gsm_internal.cuh"
+
+using namespace gsm;
+
+static thread_local std::string g_create_error;
+
+struct gsm_plan {
+    gsm_plan_desc desc{};
+    ApplyGeom geom{};
+    KrylovDims kd{};
+    KrylovState ks{};
+    cudaStream_t stream = nullptr;
+    int max_batch = 1, max_iters = 64;
+    long i0 = 0;                  // flat index of m = 0 inside one component
+    std::vector<void*> allocs;    // every device allocation, freed in destroy
+    long long device_bytes = 0, launches = 0;
+    cplx *coef = nullptr, *chat = nullptr, *W = nullptr, *xbuf = nullptr, *ybuf = nullptr;
+    double *d_kvec = nullptr, *d_k0 = nullptr, *d_resid = nullptr;
+    void* pinned = nullptr;       // host staging: nactive, iters, resid, hist
+    size_t pinned_bytes = 0;
+    mutable std::string err;
+};
+
+#define CK(call)                                                                                      \
+    do {                                                                                              \
+        cudaError_t e_ = (call);                                                                      \
+        if (e_ != cudaSuccess) {                                                                      \
+            char buf_[512];                                                                           \
+            snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return fail(plan, e_ == cudaErrorMemoryAllocation ? GSM_E_ALLOC : GSM_E_CUDA, buf_);       \
+        }                                                                                             \
+    } while (0)
+
+static gsm_status fail(const gsm_plan* plan, gsm_status st, const char* msg) {
+    if (plan) plan->err = msg; else g_create_error = msg;
+    return st;
+}
+
+template <typename T>
+static cudaError_t dalloc(gsm_plan* p, T** out, size_t count) {
+    void* q = nullptr;
+    const size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&q, bytes);
+    if (e != cudaSuccess) return e;
+    p->allocs.push_back(q);
+    p->device_bytes += (long long)bytes;
+    *out = static_cast<T*>(q);
+    return cudaSuccess;
+}
+
+static int fft_size(int N) {
+    if (N == 1) return 1;
+    int p = 1;
+    while (p < 2 * N - 1) p *= 2;
+    return p;
+}
+
+// radix plan of a power-of-two length (fft_device.cuh): larger radices last, so the fused middle stage is wide
+static bool make_axis(int P, int N, AxisPlan* ax) {
+    ax->P = P; ax->N = N; ax->nst = 0;
+    for (int i = 0; i < 4; ++i) ax->radix[i] = 1;
+    switch (P) {
+        case 1: break;
+        case 2: ax->nst = 1; ax->radix[0] = 2; break;
+        case 4: ax->nst = 1; ax->radix[0] = 4; break;
+        case 8: ax->nst = 1; ax->radix[0] = 8; break;
+        case 16: ax->nst = 2; ax->radix[0] = 4; ax->radix[1] = 4; break;
+        case 32: ax->nst = 2; ax->radix[0] = 4; ax->radix[1] = 8; break;
+        case 64: ax->nst = 2; ax->radix[0] = 8; ax->radix[1] = 8; break;
+        case 128: ax->nst = 3; ax->radix[0] = 4; ax->radix[1] = 4; ax->radix[2] = 8; break;
+        case 256: ax->nst = 3; ax->radix[0] = 4; ax->radix[1] = 8; ax->radix[2] = 8; break;
+        case 512: ax->nst = 3; ax->radix[0] = 8; ax->radix[1] = 8; ax->radix[2] = 8; break;
+        default: return false;
+    }
+    return true;
+}
+
+// position (after the forward network) of frequency k: q = k mod R0 selects block q, the rest recurses
+static int pos_of_freq(int k, int P, const int* radix, int nst) {
+    int pos = 0;
+    for (int s = 0; s < nst; ++s) {
+        const int R = radix[s];
+        P /= R;
+        pos += (k % R) * P;
+        k /= R;
+    }
+    return pos;
+}
+
+static cudaError_t upload_twiddles(gsm_plan* p, int P, const cplx** out) {
+    std::vector<double> h(2 * (size_t)P);
+    for (int k = 0; k < P; ++k) {
+        const double a = -2.0 * M_PI * (double)k / (double)P;
+        h[2 * k] = std::cos(a);
+        h[2 * k + 1] = std::sin(a);
+    }
+    // exact values on the axes
+    if (P >= 2) { h[2 * (P / 2)] = -1.0; h[2 * (P / 2) + 1] = 0.0; }
+    if (P >= 4) { h[2 * (P / 4)] = 0.0; h[2 * (P / 4) + 1] = -1.0; h[2 * (3 * P / 4)] = 0.0; h[2 * (3 * P / 4) + 1] = 1.0; }
+    cplx* d = nullptr;
+    cudaError_t e = dalloc(p, &d, (size_t)P);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpy(d, h.data(), sizeof(double) * 2 * P, cudaMemcpyHostToDevice);
+    *out = d;
+    return e;
+}
+
+static int odd_at_least(int v) { return v | 1; }
+
+static cplx cdivh(double ar, double ai, double br, double bi) {
+    const double inv = 1.0 / (br * br + bi * bi);
+    return make_double2((ar * br + ai * bi) * inv, (ai * br - ar * bi) * inv);
+}
+
+// a0: coefficients c_d on the device, either from closed forms or from an FFT of the voxel grid
+static gsm_status build_coeffs(gsm_plan* plan) {
+    const gsm_plan_desc& d = plan->desc;
+    const int* N = d.orders;
+    const size_t ncoef = (size_t)(2 * N[0] - 1) * (2 * N[1] - 1) * (2 * N[2] - 1);
+    CK(dalloc(plan, &plan->coef, ncoef));
+    if (d.eps_grid_host == nullptr) {
+        std::vector<ShapeDev> hs(std::max(d.n_shapes, 1));
+        const double vol = d.period[0] * d.period[1] * d.period[2];
+        for (int i = 0; i < d.n_shapes; ++i) {
+            const gsm_shape& s = d.shapes[i];
+            ShapeDev& q = hs[i];
+            q.kind = s.kind;
+            for (int a = 0; a < 3; ++a) { q.c[a] = s.center[a]; q.s[a] = s.size[a]; }
+            const cplx del = cdivh(s.eps_re - d.eps_bg_re, s.eps_im - d.eps_bg_im, d.eps_b_re, d.eps_b_im);
+            q.dre = del.x; q.dim = del.y;
+            if (s.kind == GSM_SPHERE) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[0] * s.size[0] / vol;
+            else if (s.kind == GSM_ELLIPSOID) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[1] * s.size[2] / vol;
+            else if (s.kind == GSM_BOX) q.f = s.size[0] * s.size[1] * s.size[2] / vol;
+            else return fail(plan, GSM_E_INVALID, "unknown shape kind");
+        }
+        ShapeDev* dsh = nullptr;
+        CK(cudaMalloc(&dsh, sizeof(ShapeDev) * hs.size()));
+        cudaError_t e = cudaMemcpyAsync(dsh, hs.data(), sizeof(ShapeDev) * hs.size(), cudaMemcpyHostToDevice, plan->stream);
+        const cplx c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_b_re, d.eps_b_im);
+        if (e == cudaSuccess) e = launch_coeffs_analytic(dsh, d.n_shapes, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
+        cudaFree(dsh);
+        CK(e);
+        return GSM_OK;
+    }
+    // voxel path: forward FFT of (eps - eps_b)/eps_b on the Nv grid, keep |d_a| <= N_a - 1
+    const int* V = d.voxels;
+    AxisPlan vax[3];
+    const cplx* vtw[3];
+    int* dpos[3] = {nullptr, nullptr, nullptr};
+    for (int a = 0; a < 3; ++a) {
+        if (V[a] < 2 * N[a] - 1 || V[a] > 512 || !make_axis(V[a], V[a], &vax[a]))
+            return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
+        CK(upload_twiddles(plan, V[a], &vtw[a]));
+        std::vector<int> pos(V[a]);
+        for (int k = 0; k < V[a]; ++k) pos[k] = pos_of_freq(k, V[a], vax[a].radix, vax[a].nst);
+        CK(dalloc(plan, &dpos[a], (size_t)V[a]));
+        CK(cudaMemcpy(dpos[a], pos.data(), sizeof(int) * V[a], cudaMemcpyHostToDevice));
+    }
+    const size_t nv = (size_t)V[0] * V[1] * V[2];
+    cplx* grid = nullptr;
+    CK(cudaMalloc(&grid, sizeof(cplx) * nv));
+    cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
+    if (e == cudaSuccess) e = launch_voxel_prepare(grid, (long)nv, d.eps_b_re, d.eps_b_im, plan->stream);
+    if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0] * V[1], vax[2], 1, vtw[2], plan->stream);
+    if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0], vax[1], V[2], vtw[1], plan->stream);
+    if (e == cudaSuccess) e = launch_fft_axis(grid, 1, vax[0], (long)V[1] * V[2], vtw[0], plan->stream);
+    if (e == cudaSuccess) e = launch_voxel_extract(grid, V, N, dpos[0], dpos[1], dpos[2], plan->coef, plan->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
+    cudaFree(grid);
+    CK(e);
+    return GSM_OK;
+}
+
+// Chat = forward network applied to the circulant embedding of c, laid out [pos3][pos1][pos2], scaled 1/(P1P2P3)
+static gsm_status build_spectrum(gsm_plan* plan) {
+    ApplyGeom& g = plan->geom;
+    const int P[3] = {g.ax[0].P, g.ax[1].P, g.ax[2].P};
+    const int N[3] = {g.N1, g.N2, g.N3};
+    const size_t np = (size_t)P[0] * P[1] * P[2];
+    CK(dalloc(plan, &plan->chat, np));
+    cplx* pad = nullptr;
+    CK(cudaMalloc(&pad, sizeof(cplx) * np));
+    cudaError_t e = launch_embed(plan->coef, N, P, pad, plan->stream);
+    AxisPlan full[3] = {g.ax[0], g.ax[1], g.ax[2]};
+    if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0] * P[1], full[2], 1, g.tw[2], plan->stream);
+    if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0], full[1], P[2], g.tw[1], plan->stream);
+    if (e == cudaSuccess) e = launch_fft_axis(pad, 1, full[0], (long)P[1] * P[2], g.tw[0], plan->stream);
+    if (e == cudaSuccess) e = launch_chat_layout(pad, P, plan->chat, plan->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
+    cudaFree(pad);
+    CK(e);
+    g.chat = plan->chat;
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out) {
+    if (out) *out = nullptr;
+    if (!desc || !out) return fail(nullptr, GSM_E_INVALID, "null descriptor or output pointer");
+    for (int a = 0; a < 3; ++a) {
+        if (desc->orders[a] < 1 || desc->orders[a] > 64) return fail(nullptr, GSM_E_INVALID, "orders must be in [1, 64]");
+        if (!(desc->period[a] > 0.0)) return fail(nullptr, GSM_E_INVALID, "periods must be positive");
+    }
+    if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(nullptr, GSM_E_INVALID, "eps_b must be non-zero");
+    if (desc->eps_grid_host == nullptr && (desc->n_shapes < 0 || (desc->n_shapes > 0 && !desc->shapes)))
+        return fail(nullptr, GSM_E_INVALID, "shapes missing");
+    gsm_plan* plan = new (std::nothrow) gsm_plan();
+    if (!plan) return fail(nullptr, GSM_E_ALLOC, "host allocation failed");
+    plan->desc = *desc;
+    plan->stream = static_cast<cudaStream_t>(desc->cuda_stream);
+    plan->max_batch = desc->max_batch > 0 ? desc->max_batch : 1;
+    plan->max_iters = desc->max_iters > 0 ? desc->max_iters : 64;
+    gsm_status st = GSM_OK;
+    auto body = [&]() -> gsm_status {
+        ApplyGeom& g = plan->geom;
+        const int* N = desc->orders;
+        g.N1 = N[0]; g.N2 = N[1]; g.N3 = N[2];
+        g.NL = N[0] * N[1];
+        g.n = (long)N[0] * N[1] * N[2];
+        for (int a = 0; a < 3; ++a) {
+            if (!make_axis(fft_size(N[a]), N[a], &g.ax[a])) return fail(plan, GSM_E_INVALID, "unsupported FFT size");
+            g.K[a] = 2.0 * M_PI / desc->period[a];
+            g.mmin[a] = (N[a] % 2 == 1) ? -(N[a] - 1) / 2 : -N[a] / 2;
+            CK(upload_twiddles(plan, g.ax[a].P, &g.tw[a]));
+        }
+        g.epsb_re = desc->eps_b_re; g.epsb_im = desc->eps_b_im;
+        g.L = std::min(g.NL, g.ax[2].P >= 128 ? 16 : 32);
+        g.Lst = odd_at_least(g.L);
+        g.RS3 = odd_at_least(3 * g.L);
+        g.N1s = odd_at_least(g.N1);
+        g.CB = std::min(g.ax[1].P, g.ax[0].P >= 128 ? 16 : 32);
+        g.CBs = odd_at_least(g.CB);
+        if (apply_smem_max(g) > 227 * 1024) return fail(plan, GSM_E_INVALID, "orders too large for the shared-memory tiles");
+        plan->i0 = ((long)(-g.mmin[0]) * N[1] + (-g.mmin[1])) * N[2] + (-g.mmin[2]);
+        CK(apply_init_attributes());
+        CK(plan_init_attributes());
+        CK(krylov_init_attributes());
+        gsm_status s2 = build_coeffs(plan);
+        if (s2 != GSM_OK) return s2;
+        s2 = build_spectrum(plan);
+        if (s2 != GSM_OK) return s2;
+        // workspaces
+        const int B = plan->max_batch, m = plan->max_iters;
+        KrylovDims& kd = plan->kd;
+        kd.vlen = 3 * g.n;
+        kd.chunk = 256 * 4;
+        kd.nchunk = (int)((kd.vlen + kd.chunk - 1) / kd.chunk);
+        kd.mmax = m;
+        kd.ld = m + 1;
+        KrylovState& ks = plan->ks;
+        CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
+        CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
+        CK(dalloc(plan, &plan->ybuf, (size_t)B * kd.vlen));
+        CK(dalloc(plan, &ks.basis, (size_t)kd.ld * B * kd.vlen));
+        CK(dalloc(plan, &ks.part, (size_t)B * kd.nchunk * 2 * kd.ld));
+        CK(dalloc(plan, &ks.gram, (size_t)B * kd.ld * kd.ld));
+        CK(dalloc(plan, &ks.hcol, (size_t)B * kd.ld));
+        CK(dalloc(plan, &ks.R, (size_t)B * kd.ld * kd.mmax));
+        CK(dalloc(plan, &ks.cs, (size_t)B * kd.mmax));
+        CK(dalloc(plan, &ks.sn, (size_t)B * kd.mmax));
+        CK(dalloc(plan, &ks.g, (size_t)B * kd.ld));
+        CK(dalloc(plan, &ks.ycoef, (size_t)B * kd.mmax));
+        CK(dalloc(plan, &ks.hist, (size_t)B * kd.mmax));
+        CK(dalloc(plan, &ks.beta, (size_t)B));
+        CK(dalloc(plan, &ks.scale, (size_t)B));
+        CK(dalloc(plan, &ks.active, (size_t)B));
+        CK(dalloc(plan, &ks.iters, (size_t)B));
+        CK(dalloc(plan, &ks.nactive, (size_t)1));
+        CK(dalloc(plan, &ks.pol, (size_t)B * 6));
+        CK(dalloc(plan, &ks.tol, (size_t)1));
+        CK(dalloc(plan, &plan->d_kvec, (size_t)B * 3));
+        CK(dalloc(plan, &plan->d_k0, (size_t)B));
+        CK(dalloc(plan, &plan->d_resid, (size_t)B));
+        plan->pinned_bytes = sizeof(double) * ((size_t)B * (12 + kd.mmax) + 16);
+        CK(cudaMallocHost(&plan->pinned, plan->pinned_bytes));
+        return GSM_OK;
+    };
+    st = body();
+    if (st != GSM_OK) {
+        g_create_error = plan->err;
+        gsm_plan_destroy(plan);
+        return st;
+    }
+    *out = plan;
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
+    if (!plan) return GSM_E_INVALID;
+    cudaStreamSynchronize(plan->stream);
+    for (void* p : plan->allocs) cudaFree(p);
+    if (plan->pinned) cudaFreeHost(plan->pinned);
+    delete plan;
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_plan_coeffs(const gsm_plan* plan, double* host_out) {
+    if (!plan || !host_out) return GSM_E_INVALID;
+    const int* N = plan->desc.orders;
+    const size_t ncoef = (size_t)(2 * N[0] - 1) * (2 * N[1] - 1) * (2 * N[2] - 1);
+    CK(cudaStreamSynchronize(plan->stream));
+    CK(cudaMemcpy(host_out, plan->coef, sizeof(cplx) * ncoef, cudaMemcpyDeviceToHost));
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_plan_info(const gsm_plan* plan, int fft_grid[3], long long* device_bytes, long long* launches) {
+    if (!plan) return GSM_E_INVALID;
+    if (fft_grid) for (int a = 0; a < 3; ++a) fft_grid[a] = plan->geom.ax[a].P;
+    if (device_bytes) *device_bytes = plan->device_bytes;
+    if (launches) *launches = plan->launches;
+    return GSM_OK;
+}
+
+extern "C" const char* gsm_last_error(const gsm_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+// eps_b must keep k_m.k_m != k_b^2 for every kept m.  min over m of |k_m.k_m - k_b^2| / |k_b^2| on the
+// host: k_m.k_m = a1(m1) + a2(m2) + a3(m3) is separable, so a sorted a3 and a binary search give O(N1 N2 log N3).
+static bool singular_basis(const gsm_plan* plan, int batch, const double* kvec, const double* k0) {
+    const ApplyGeom& g = plan->geom;
+    const int N[3] = {g.N1, g.N2, g.N3};
+    std::vector<double> a[3];
+    for (int b = 0; b < batch; ++b) {
+        const double kb2r = k0[b] * k0[b] * g.epsb_re, kb2i = k0[b] * k0[b] * g.epsb_im;
+        const double mag = std::hypot(kb2r, kb2i);
+        for (int ax = 0; ax < 3; ++ax) {
+            a[ax].resize(N[ax]);
+            for (int i = 0; i < N[ax]; ++i) {
+                const double k = kvec[3 * b + ax] + (i + g.mmin[ax]) * g.K[ax];
+                a[ax][i] = k * k;
+            }
+        }
+        std::sort(a[2].begin(), a[2].end());
+        double best = INFINITY;
+        for (int i = 0; i < N[0]; ++i)
+            for (int j = 0; j < N[1]; ++j) {
+                const double target = kb2r - a[0][i] - a[1][j];
+                auto it = std::lower_bound(a[2].begin(), a[2].end(), target);
+                if (it != a[2].end()) best = std::min(best, std::fabs(*it - target));
+                if (it != a[2].begin()) best = std::min(best, std::fabs(*(it - 1) - target));
+            }
+        const double dist = std::hypot(best, kb2i);
+        if (!(dist > 1e-12 * mag) || !std::isfinite(dist)) return true;
+    }
+    return false;
+}
+
+extern "C" gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch, const double* k0, const void* d_x,
+                                void* d_y) {
+    if (!plan) return GSM_E_INVALID;
+    if (!k_bloch || !k0 || !d_x || !d_y || batch < 1 || batch > plan->max_batch || d_x == d_y)
+        return fail(plan, GSM_E_INVALID, "gsm_apply: bad argument");
+    if (singular_basis(plan, batch, k_bloch, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
+    CK(cudaMemcpyAsync(plan->d_kvec, k_bloch, sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, plan->stream));
+    CK(cudaMemcpyAsync(plan->d_k0, k0, sizeof(double) * batch, cudaMemcpyHostToDevice, plan->stream));
+    CK(launch_apply(plan->geom, batch, plan->d_kvec, plan->d_k0, static_cast<const cplx*>(d_x), static_cast<cplx*>(d_y),
+                    plan->W, nullptr, plan->stream, &plan->launches));
+    return GSM_OK;
+}
+
+// nb <= max_batch solves in lock step.  d_E: device [nb][vlen].  Host outputs may be null.
+static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const double* k0, const double* pol, double tol,
+                            cplx* d_E, double* resp, int* iters, double* resid, double* hist, int hist_cap,
+                            bool* not_converged) {
+    const KrylovDims& kd = plan->kd;
+    const KrylovState& ks = plan->ks;
+    const ApplyGeom& g = plan->geom;
+    cudaStream_t st = plan->stream;
+    if (singular_basis(plan, nb, kvec, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
+    double* pin = static_cast<double*>(plan->pinned);
+    int* pin_i = reinterpret_cast<int*>(pin);           // [0] nactive; then staging
+    CK(cudaMemcpyAsync(plan->d_kvec, kvec, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(plan->d_k0, k0, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ks.pol, pol, sizeof(double) * 6 * nb, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ks.tol, &tol, sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ks.nactive, &nb, sizeof(int), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(ks.basis, 0, sizeof(cplx) * (size_t)nb * kd.vlen, st));
+    CK(launch_krylov_init(kd, ks, nb, plan->i0, g.n, st));
+    plan->launches += 1;
+    const size_t vs = (size_t)nb * kd.vlen;
+    int j = 0;
+    for (; j < kd.mmax; ++j) {
+        CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
+                        plan->W, ks.active, st, &plan->launches));
+        CK(launch_sweep_dots(kd, ks, nb, j, st));
+        CK(launch_hsolve(kd, ks, nb, j, st));
+        CK(launch_sweep_update(kd, ks, nb, j, st));
+        CK(launch_givens(kd, ks, nb, j, st));
+        CK(launch_normalize(kd, ks, nb, j, st));
+        plan->launches += 5;
+        CK(cudaMemcpyAsync(pin_i, ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (pin_i[0] <= 0) break;
+    }
+    CK(launch_backsolve(kd, ks, nb, st));
+    CK(launch_combine(kd, ks, nb, d_E, st));
+    // true residual with one more apply
+    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, nullptr, st, &plan->launches));
+    CK(launch_true_residual(kd, ks, nb, plan->ybuf, plan->i0, g.n, plan->d_resid, st));
+    plan->launches += 4;
+    int* h_iters = reinterpret_cast<int*>(pin + 2);
+    double* h_resid = pin + 2 + nb;           // ints occupy at most nb doubles
+    int* h_active = reinterpret_cast<int*>(pin + 2 + 2 * (size_t)nb);
+    double* h_resp = pin + 2 + 3 * (size_t)nb;
+    CK(cudaMemcpyAsync(h_iters, ks.iters, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_resid, plan->d_resid, sizeof(double) * nb, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_active, ks.active, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+    // E at m = 0: three complex numbers per solve, stride n inside a vector
+    CK(cudaMemcpy2DAsync(h_resp, sizeof(cplx), d_E + plan->i0, sizeof(cplx) * g.n, sizeof(cplx), (size_t)3 * nb,
+                         cudaMemcpyDeviceToHost, st));
+    if (hist && hist_cap > 0)
+        CK(cudaMemcpyAsync(pin + 2 + 9 * (size_t)nb, ks.hist, sizeof(double) * std::min(hist_cap, kd.mmax),
+                           cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    for (int b = 0; b < nb; ++b) {
+        if (iters) iters[b] = h_iters[b];
+        if (resid) resid[b] = h_resid[b];
+        if (h_active[b]) *not_converged = true;
+        if (resp) for (int q = 0; q < 6; ++q) resp[6 * b + q] = h_resp[6 * b + q];
+    }
+    if (hist && hist_cap > 0) {
+        const int cnt = std::min(std::min(hist_cap, kd.mmax), h_iters[0]);
+        for (int q = 0; q < cnt; ++q) hist[q] = pin[2 + 9 * (size_t)nb + q];
+    }
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double k0, const double pol[6], double tol,
+                                void* d_E_out, double* resid_hist_host, int hist_cap, int* n_iters,
+                                double* true_rel_resid) {
+    if (!plan) return GSM_E_INVALID;
+    if (!k_bloch || !pol || !d_E_out || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_solve: bad argument");
+    bool nc = false;
+    gsm_status s = run_batch(plan, 1, k_bloch, &k0, pol, tol, static_cast<cplx*>(d_E_out), nullptr, n_iters,
+                             true_rel_resid, resid_hist_host, hist_cap, &nc);
+    if (s != GSM_OK) return s;
+    return nc ? GSM_NOT_CONVERGED : GSM_OK;
+}
+
+extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                               double tol, double* resp_host, int* iters, double* resid, void* d_E_out) {
+    if (!plan) return GSM_E_INVALID;
+    if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_scan: bad argument");
+    bool nc = false;
+    for (int p0 = 0; p0 < npts; p0 += plan->max_batch) {
+        const int nb = std::min(plan->max_batch, npts - p0);
+        cplx* dE = d_E_out ? static_cast<cplx*>(d_E_out) + (size_t)p0 * plan->kd.vlen : plan->xbuf;
+        gsm_status s = run_batch(plan, nb, k_bloch + 3 * (size_t)p0, k0 + p0, pol + 6 * (size_t)p0, tol, dE,
+                                 resp_host ? resp_host + 6 * (size_t)p0 : nullptr, iters ? iters + p0 : nullptr,
+                                 resid ? resid + p0 : nullptr, nullptr, 0, &nc);
+        if (s != GSM_OK) return s;
+    }
+    return nc ? GSM_NOT_CONVERGED : GSM_OK;
+}

@@ -1,0 +1,97 @@
+// gsm_internal.cuh - shared declarations of the CUDA library behind include/gsm.h (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+
+#include "fft_device.cuh"
+#include "gsm.h"
+
+namespace gsm {
+
+// Geometry of the operator apply shared by the three passes.
+struct ApplyGeom {
+    AxisPlan ax[3];      // x, y, z axes of the circulant grid
+    int N1, N2, N3;      // harmonics kept
+    int NL;              // N1*N2 = number of z-lines per component
+    long n;              // N1*N2*N3
+    int L;               // z-lines per CTA in passes 1 and 3
+    int Lst;             // odd row stride (>= L) of the pass-1 tile
+    int RS3;             // odd row stride (>= 3L) of the pass-3 tile
+    int N1s;             // odd row stride (>= N1) of the pass-2 plane
+    int CB, CBs;         // columns per x-batch in pass 2 and the odd row stride (>= CB) of its scratch
+    const cplx* tw[3];   // device twiddle tables exp(-2 pi i k / P_a)
+    const cplx* chat;    // coefficient spectrum, position order, [P3][P1][P2], scaled by 1/(P1 P2 P3)
+    double K[3];         // 2 pi / Lambda_a
+    int mmin[3];         // lowest order per axis
+    double epsb_re, epsb_im;
+};
+
+struct KrylovDims {
+    long vlen;       // 3n complex numbers per vector
+    int nchunk;      // CTAs per vector in the sweeps
+    int chunk;       // elements per CTA (= threads * elems per thread)
+    int mmax;        // max iterations (basis holds mmax+1 vectors)
+    int ld;          // mmax + 1
+};
+
+// ---- launches implemented in apply.cu --------------------------------------------------------------------------
+// y[b] = x[b] - G_b (T x[b]); kvec[b][3], k0[b] device arrays; W workspace [batch][3][P3][NL].
+// active (may be null): per-solve flags; CTAs of solves with active[b] == 0 exit at once.
+cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
+                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, long long* launches);
+size_t apply_smem_max(const ApplyGeom& g);
+cudaError_t apply_init_attributes();
+cudaError_t plan_init_attributes();
+
+// plan-time (a0): coefficients and their spectrum
+struct ShapeDev {
+    int kind;
+    double c[3], s[3], dre, dim;  // centre, size, (eps_i - eps_bg)/eps_b
+    double f;                     // volume fraction
+};
+cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, double c0_re, double c0_im, const double K[3],
+                                   const int N[3], cplx* d_coef, cudaStream_t st);
+// generic forward FFT along one axis of a dense [outer][P][inner] complex array in global memory (plan time only)
+cudaError_t launch_fft_axis(cplx* d_data, long outer, const AxisPlan& ax, long inner, const cplx* d_tw, cudaStream_t st);
+cudaError_t launch_embed(const cplx* d_coef, const int N[3], const int P[3], cplx* d_pad, cudaStream_t st);
+cudaError_t launch_chat_layout(const cplx* d_padfft, const int P[3], cplx* d_chat, cudaStream_t st);
+cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, cudaStream_t st);
+cudaError_t launch_voxel_extract(const cplx* d_gridfft, const int Nv[3], const int N[3], const int* d_pos1,
+                                 const int* d_pos2, const int* d_pos3, cplx* d_coef, cudaStream_t st);
+
+// ---- launches implemented in krylov.cu -------------------------------------------------------------------------
+struct KrylovState {   // all device pointers, one entry (or row) per solve of the batch
+    cplx* basis;       // [ld][batch][vlen]
+    cplx* part;        // [batch][nchunk][2*ld] partial inner products of sweep 1 / partial norms of sweep 2
+    cplx* gram;        // [batch][ld][ld]   gram[j][i] = <v_i, v_j>, i <= j
+    cplx* hcol;        // [batch][ld]       current Hessenberg column after Gram-Schmidt
+    cplx* R;           // [batch][ld][mmax] rotated Hessenberg (upper triangular)
+    double* cs;        // [batch][mmax]
+    cplx* sn;          // [batch][mmax]
+    cplx* g;           // [batch][ld]
+    cplx* ycoef;       // [batch][mmax]
+    double* hist;      // [batch][mmax]
+    double* beta;      // [batch]
+    double* scale;     // [batch] 1 / h_{j+1,j} of the running iteration
+    int* active;       // [batch] 1 while iterating
+    int* iters;        // [batch]
+    int* nactive;      // [1]
+    double* pol;       // [batch][6]
+    double* tol;       // [1]
+};
+cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0 /*index of m=0*/, long n,
+                               cudaStream_t st);
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
+cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
+cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st);
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st);
+// resid[b] = || pol delta_m0 - y[b] || / beta[b]
+cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
+                                 double* d_resid, cudaStream_t st);
+cudaError_t krylov_init_attributes();
+
+}  // namespace gsm

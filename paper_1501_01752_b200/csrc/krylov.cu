@@ -1,0 +1,376 @@
+// krylov.cu - batched lock-step GMRES ("GMRes ... according to Saad with the modified
+// Gram-Schmidt orthogonalization"), one instance per (k, omega) point of the scan, all device-resident.
+//
+// Gram-Schmidt.  Saad's MGS step is  h_i = <v_i, w - sum_{k<i} h_k v_k>, i = 0..j.  Expanding the inner product,
+//     h_i = <v_i, w> - sum_{k<i} h_k <v_i, v_k>,
+// an identity that needs no orthogonality assumption.  So one streaming sweep over the basis gives every
+// <v_i, w> together with the new row <v_i, v_j> of the Gram matrix (sweep_dots), a tiny per-solve recurrence
+// gives the same h_i MGS produces up to rounding order (hsolve), and a second streaming sweep forms
+// w - sum h_i v_i and its norm (sweep_update).  This replaces the paper's one-CUBLAS-call-per-dot/axpy (5 vector
+// passes per basis vector, j grid-wide reductions per iteration) by 2 passes per basis vector and 2 reductions.
+// The paper's library calls were made for a GTX Titan; the algebra is kept, the schedule is not.
+//
+// <u, v> = sum conj(u) v.  Reductions are two-stage and deterministic (per-CTA partials, then a fixed-order sum).
+#include "gsm_internal.cuh"
+
+namespace gsm {
+
+#define KT 256   // threads per CTA in the sweeps
+
+static __device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void krylov_init_kernel(KrylovDims d, KrylovState s, int batch, long i0, long n) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const double* p = s.pol + 6 * b;
+    const double beta = sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3] + p[4] * p[4] + p[5] * p[5]);
+    s.beta[b] = beta;
+    s.iters[b] = 0;
+    s.active[b] = beta > 0.0 ? 1 : 0;
+    if (beta <= 0.0) atomicSub(s.nactive, 1);
+    for (int i = 0; i < d.ld; ++i) s.g[(long)b * d.ld + i] = make_double2(0.0, 0.0);
+    s.g[(long)b * d.ld] = make_double2(beta, 0.0);
+    if (beta > 0.0) {
+        cplx* v0 = s.basis + (long)b * d.vlen;
+        for (int c = 0; c < 3; ++c) v0[c * n + i0] = make_double2(p[2 * c] / beta, p[2 * c + 1] / beta);
+    }
+}
+
+// sweep 1: part[b][chunk][2i] = sum_chunk conj(v_i) w, part[..][2i+1] = sum_chunk conj(v_i) v_j, i = 0..j
+template <int E>
+__global__ void __launch_bounds__(KT) sweep_dots_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+    const int b = blockIdx.y;
+    if (!s.active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* red = reinterpret_cast<double*>(smem_raw);   // [KT/32][j+1][4]
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    const long vs = (long)batch * d.vlen;
+    const cplx* vb = s.basis + (long)b * d.vlen;
+    const cplx* w = vb + (long)(j + 1) * vs;
+    const cplx* vj = vb + (long)j * vs;
+    cplx wr[E], vr[E];
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        const bool ok = e < d.vlen;
+        wr[k] = ok ? w[e] : make_double2(0.0, 0.0);
+        vr[k] = ok ? vj[e] : make_double2(0.0, 0.0);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = 0; i <= j; ++i) {
+        const cplx* vi = vb + (long)i * vs;
+        cplx u[E];
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            const long e = e0 + (long)k * KT;
+            u[k] = (e < d.vlen) ? vi[e] : make_double2(0.0, 0.0);
+        }
+        double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
+#pragma unroll
+        for (int k = 0; k < E; ++k) {   // conj(u) * w, conj(u) * vj
+            a0 = fma(u[k].x, wr[k].x, fma(u[k].y, wr[k].y, a0));
+            a1 = fma(u[k].x, wr[k].y, fma(-u[k].y, wr[k].x, a1));
+            g0 = fma(u[k].x, vr[k].x, fma(u[k].y, vr[k].y, g0));
+            g1 = fma(u[k].x, vr[k].y, fma(-u[k].y, vr[k].x, g1));
+        }
+        a0 = warp_sum(a0); a1 = warp_sum(a1); g0 = warp_sum(g0); g1 = warp_sum(g1);
+        if (lane == 0) {
+            double* r = red + ((long)warp * (j + 1) + i) * 4;
+            r[0] = a0; r[1] = a1; r[2] = g0; r[3] = g1;
+        }
+    }
+    __syncthreads();
+    cplx* out = s.part + ((long)b * d.nchunk + blockIdx.x) * 2 * d.ld;
+    for (int i = threadIdx.x; i <= j; i += KT) {
+        double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
+        for (int wq = 0; wq < KT / 32; ++wq) {
+            const double* r = red + ((long)wq * (j + 1) + i) * 4;
+            a0 += r[0]; a1 += r[1]; g0 += r[2]; g1 += r[3];
+        }
+        out[2 * i] = make_double2(a0, a1);
+        out[2 * i + 1] = make_double2(g0, g1);
+    }
+}
+
+// per solve: reduce the partials, store the Gram row, run the MGS recurrence -> hcol[0..j]
+__global__ void __launch_bounds__(32) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+    const int b = blockIdx.x;
+    if (!s.active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* dd = reinterpret_cast<cplx*>(smem_raw);   // [ld]
+    cplx* gT = s.gram + (long)b * d.ld * d.ld;      // gT[k*ld + i] = <v_k, v_i>, k <= i
+    const int lane = threadIdx.x;
+    for (int i = lane; i <= j; i += 32) {
+        double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
+        const cplx* p = s.part + (long)b * d.nchunk * 2 * d.ld + 2 * i;
+        for (int c = 0; c < d.nchunk; ++c) {
+            const cplx a = p[(long)c * 2 * d.ld], g = p[(long)c * 2 * d.ld + 1];
+            a0 += a.x; a1 += a.y; g0 += g.x; g1 += g.y;
+        }
+        dd[i] = make_double2(a0, a1);
+        gT[(long)i * d.ld + j] = make_double2(g0, g1);
+    }
+    __syncwarp();
+    // column-oriented recurrence: once h_k is final, every later d_i loses h_k <v_i, v_k> = h_k conj(<v_k, v_i>)
+    for (int k = 0; k < j; ++k) {
+        const cplx hk = dd[k];
+        for (int i = k + 1 + lane; i <= j; i += 32) {
+            const cplx gki = gT[(long)k * d.ld + i];
+            const cplx t = cmulc(hk, gki);
+            dd[i] = make_double2(dd[i].x - t.x, dd[i].y - t.y);
+        }
+        __syncwarp();
+    }
+    for (int i = lane; i <= j; i += 32) s.hcol[(long)b * d.ld + i] = dd[i];
+}
+
+// sweep 2: w <- w - sum_i h_i v_i ; npart[b][chunk] = sum_chunk |w|^2   (stored in part[b][chunk][0].x)
+template <int E>
+__global__ void __launch_bounds__(KT) sweep_update_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+    const int b = blockIdx.y;
+    if (!s.active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* h = reinterpret_cast<cplx*>(smem_raw);   // [j+1]
+    __shared__ double wsum[KT / 32];
+    for (int i = threadIdx.x; i <= j; i += KT) h[i] = s.hcol[(long)b * d.ld + i];
+    __syncthreads();
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    const long vs = (long)batch * d.vlen;
+    const cplx* vb = s.basis + (long)b * d.vlen;
+    cplx* w = s.basis + (long)b * d.vlen + (long)(j + 1) * vs;
+    cplx wr[E];
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        wr[k] = (e < d.vlen) ? w[e] : make_double2(0.0, 0.0);
+    }
+    for (int i = 0; i <= j; ++i) {
+        const cplx* vi = vb + (long)i * vs;
+        const cplx hi = h[i];
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            const long e = e0 + (long)k * KT;
+            const cplx u = (e < d.vlen) ? vi[e] : make_double2(0.0, 0.0);
+            wr[k].x = fma(-hi.x, u.x, fma(hi.y, u.y, wr[k].x));
+            wr[k].y = fma(-hi.x, u.y, fma(-hi.y, u.x, wr[k].y));
+        }
+    }
+    double nn = 0.0;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) {
+            w[e] = wr[k];
+            nn = fma(wr[k].x, wr[k].x, fma(wr[k].y, wr[k].y, nn));
+        }
+    }
+    nn = warp_sum(nn);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = nn;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int q = 0; q < KT / 32; ++q) t += wsum[q];
+        s.part[((long)b * d.nchunk + blockIdx.x) * 2 * d.ld] = make_double2(t, 0.0);
+    }
+}
+
+// per solve: h_{j+1,j} = ||w||, Givens least squares (Saad Alg. 6.9 / 6.5.3), residual estimate, stop test
+__global__ void givens_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch || !s.active[b]) return;
+    double nn = 0.0;
+    for (int c = 0; c < d.nchunk; ++c) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    const double hn = sqrt(nn);
+    cplx* Rc = s.R + (long)b * d.ld * d.mmax;     // Rc[i * mmax + j]
+    const cplx* h = s.hcol + (long)b * d.ld;
+    double* cs = s.cs + (long)b * d.mmax;
+    cplx* sn = s.sn + (long)b * d.mmax;
+    cplx* g = s.g + (long)b * d.ld;
+    cplx hi = h[0];
+    for (int i = 0; i < j; ++i) {   // previous rotations on the new column
+        const cplx hn1 = h[i + 1];
+        const cplx t = cadd(make_double2(cs[i] * hi.x, cs[i] * hi.y), cmul(sn[i], hn1));
+        const cplx u = csub(make_double2(cs[i] * hn1.x, cs[i] * hn1.y), cmulc(hi, sn[i]));   // -conj(sn) hi + cs hn1
+        Rc[(long)i * d.mmax + j] = t;
+        hi = u;
+    }
+    const cplx a = hi;
+    const double aa = hypot(a.x, a.y);
+    const double r = hypot(aa, hn);
+    double c;
+    cplx sv;
+    if (r == 0.0) { c = 1.0; sv = make_double2(0.0, 0.0); }
+    else if (aa == 0.0) { c = 0.0; sv = make_double2(1.0, 0.0); }
+    else { c = aa / r; sv = make_double2(a.x / aa * hn / r, a.y / aa * hn / r); }   // (a/|a|) conj(hn)/r, hn real
+    cs[j] = c;
+    sn[j] = sv;
+    Rc[(long)j * d.mmax + j] = cadd(make_double2(c * a.x, c * a.y), make_double2(sv.x * hn, sv.y * hn));
+    const cplx gj = g[j];
+    g[j + 1] = make_double2(-(sv.x * gj.x + sv.y * gj.y), -(sv.x * gj.y - sv.y * gj.x));   // -conj(sn) g_j
+    g[j] = make_double2(c * gj.x, c * gj.y);
+    const double beta = s.beta[b];
+    const double res = hypot(g[j + 1].x, g[j + 1].y) / beta;
+    s.hist[(long)b * d.mmax + j] = res;
+    s.iters[b] = j + 1;
+    const bool lucky = hn <= 2.220446049250313e-16 * beta;
+    if (res <= s.tol[0] || lucky) {
+        s.active[b] = 0;
+        atomicSub(s.nactive, 1);
+    } else {
+        s.scale[b] = 1.0 / hn;
+    }
+}
+
+// v_{j+1} = w / h_{j+1,j}
+template <int E>
+__global__ void __launch_bounds__(KT) normalize_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+    const int b = blockIdx.y;
+    if (!s.active[b]) return;
+    const double sc = s.scale[b];
+    cplx* w = s.basis + (long)b * d.vlen + (long)(j + 1) * batch * d.vlen;
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) {
+            const cplx v = w[e];
+            w[e] = make_double2(v.x * sc, v.y * sc);
+        }
+    }
+}
+
+// y = R^{-1} g (upper triangular, m = iters[b])
+__global__ void backsolve_kernel(KrylovDims d, KrylovState s, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const int m = s.iters[b];
+    const cplx* Rc = s.R + (long)b * d.ld * d.mmax;
+    const cplx* g = s.g + (long)b * d.ld;
+    cplx* y = s.ycoef + (long)b * d.mmax;
+    for (int i = m - 1; i >= 0; --i) {
+        cplx acc = g[i];
+        for (int k = i + 1; k < m; ++k) acc = csub(acc, cmul(Rc[(long)i * d.mmax + k], y[k]));
+        const cplx rii = Rc[(long)i * d.mmax + i];
+        const double inv = 1.0 / (rii.x * rii.x + rii.y * rii.y);
+        y[i] = make_double2((acc.x * rii.x + acc.y * rii.y) * inv, (acc.y * rii.x - acc.x * rii.y) * inv);
+    }
+}
+
+// E[b] = sum_{i<m} y_i v_i
+template <int E>
+__global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s, int batch, cplx* __restrict__ out) {
+    const int b = blockIdx.y;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* y = reinterpret_cast<cplx*>(smem_raw);
+    const int m = s.iters[b];
+    for (int i = threadIdx.x; i < m; i += KT) y[i] = s.ycoef[(long)b * d.mmax + i];
+    __syncthreads();
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    const long vs = (long)batch * d.vlen;
+    const cplx* vb = s.basis + (long)b * d.vlen;
+    cplx acc[E];
+#pragma unroll
+    for (int k = 0; k < E; ++k) acc[k] = make_double2(0.0, 0.0);
+    for (int i = 0; i < m; ++i) {
+        const cplx* vi = vb + (long)i * vs;
+        const cplx yi = y[i];
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            const long e = e0 + (long)k * KT;
+            if (e < d.vlen) acc[k] = cfma(yi, vi[e], acc[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) out[(long)b * d.vlen + e] = acc[k];
+    }
+}
+
+// partial ||b - y||^2 per chunk, b = pol delta_{m,0}
+template <int E>
+__global__ void __launch_bounds__(KT) resid_part_kernel(KrylovDims d, KrylovState s, int batch, const cplx* __restrict__ y,
+                                                        long i0, long n) {
+    const int b = blockIdx.y;
+    __shared__ double wsum[KT / 32];
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    double nn = 0.0;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) {
+            cplx v = y[(long)b * d.vlen + e];
+            const long c = e / n, r = e - c * n;
+            if (r == i0) { v.x -= s.pol[6 * b + 2 * c]; v.y -= s.pol[6 * b + 2 * c + 1]; }
+            nn = fma(v.x, v.x, fma(v.y, v.y, nn));
+        }
+    }
+    nn = warp_sum(nn);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = nn;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int q = 0; q < KT / 32; ++q) t += wsum[q];
+        s.part[((long)b * d.nchunk + blockIdx.x) * 2 * d.ld] = make_double2(t, 0.0);
+    }
+}
+__global__ void resid_final_kernel(KrylovDims d, KrylovState s, int batch, double* __restrict__ resid) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    double nn = 0.0;
+    for (int c = 0; c < d.nchunk; ++c) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    resid[b] = s.beta[b] > 0.0 ? sqrt(nn) / s.beta[b] : 0.0;
+}
+
+// ---- host-side launchers ----------------------------------------------------------------------------------------
+#define GSM_E 4   // elements per thread in the sweeps (KrylovDims.chunk = KT * GSM_E)
+
+cudaError_t krylov_init_attributes() {
+    cudaError_t e = cudaFuncSetAttribute(sweep_dots_kernel<GSM_E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    return e;
+}
+cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st) {
+    krylov_init_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, i0, n);
+    return cudaGetLastError();
+}
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+    const size_t smem = sizeof(double) * 4 * (KT / 32) * (size_t)(j + 1);
+    sweep_dots_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, smem, st>>>(d, s, batch, j);
+    return cudaGetLastError();
+}
+cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+    hsolve_kernel<<<batch, 32, sizeof(cplx) * d.ld, st>>>(d, s, batch, j);
+    return cudaGetLastError();
+}
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+    sweep_update_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * (j + 1), st>>>(d, s, batch, j);
+    return cudaGetLastError();
+}
+cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+    givens_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch, j);
+    return cudaGetLastError();
+}
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+    normalize_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, j);
+    return cudaGetLastError();
+}
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st) {
+    backsolve_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch);
+    return cudaGetLastError();
+}
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st) {
+    combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_E);
+    return cudaGetLastError();
+}
+cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
+                                 double* d_resid, cudaStream_t st) {
+    resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, d_y, i0, n);
+    resid_final_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, d_resid);
+    return cudaGetLastError();
+}
+
+}  // namespace gsm

@@ -1,0 +1,218 @@
+"""Thin ctypes binding of the C ABI in include/gsm.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA library ``libgsm_b200.so``; PyTorch is used for device memory and
+the stream.  Importing this module fails loudly if the library has not been built - there is no CPU fallback.
+Names follow include/gsm.h: Plan.apply / solve / scan and pole_search map 1:1 to gsm_apply / gsm_solve /
+gsm_scan / gsm_pole_search.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgsm_b200.so")
+
+OK, NOT_CONVERGED, E_INVALID, E_ALLOC, E_CUDA, E_SINGULAR_BASIS = 0, 1, -1, -2, -3, -4
+SPHERE, ELLIPSOID, BOX = 0, 1, 2
+
+
+class GsmError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"gsm status {status}: {msg}")
+        self.status = status
+
+
+class _Shape(C.Structure):
+    _fields_ = [("kind", C.c_int), ("center", C.c_double * 3), ("size", C.c_double * 3),
+                ("eps_re", C.c_double), ("eps_im", C.c_double)]
+
+
+class _PlanDesc(C.Structure):
+    _fields_ = [("period", C.c_double * 3), ("orders", C.c_int * 3),
+                ("eps_bg_re", C.c_double), ("eps_bg_im", C.c_double),
+                ("eps_b_re", C.c_double), ("eps_b_im", C.c_double),
+                ("n_shapes", C.c_int), ("shapes", C.POINTER(_Shape)),
+                ("voxels", C.c_int * 3), ("eps_grid_host", C.c_void_p),
+                ("max_iters", C.c_int), ("max_batch", C.c_int), ("cuda_stream", C.c_void_p)]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'`. "
+                          "There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    P = C.c_void_p
+    dp = C.POINTER(C.c_double)
+    ip = C.POINTER(C.c_int)
+    lib.gsm_plan_create.argtypes = [C.POINTER(_PlanDesc), C.POINTER(P)]
+    lib.gsm_plan_destroy.argtypes = [P]
+    lib.gsm_plan_coeffs.argtypes = [P, P]
+    lib.gsm_plan_info.argtypes = [P, ip, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    lib.gsm_apply.argtypes = [P, C.c_int, P, P, P, P]
+    lib.gsm_solve.argtypes = [P, P, C.c_double, P, C.c_double, P, P, C.c_int, ip, dp]
+    lib.gsm_scan.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P]
+    lib.gsm_pole_search.argtypes = [C.c_int, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P, ip]
+    lib.gsm_last_error.argtypes = [P]
+    lib.gsm_last_error.restype = C.c_char_p
+    for f in ("gsm_plan_create", "gsm_plan_destroy", "gsm_plan_coeffs", "gsm_plan_info", "gsm_apply", "gsm_solve",
+              "gsm_scan", "gsm_pole_search"):
+        getattr(lib, f).restype = C.c_int
+    return lib
+
+
+_lib = _load()
+
+
+def _f64(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def _check(status, plan=None, allow_warning=True):
+    if status < 0 or (status > 0 and not allow_warning):
+        msg = _lib.gsm_last_error(plan).decode() if True else ""
+        raise GsmError(status, msg)
+    return status
+
+
+class Plan:
+    """gsm_plan: one periodic cell (periods, orders, shapes or voxel grid) on the current CUDA device."""
+
+    def __init__(self, periods, orders, shapes=None, eps_bg=1.0, eps_b=None, voxels=None, max_iters=64, max_batch=1,
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1501_01752_b200.gsm needs a CUDA device; there is no CPU fallback")
+        self._torch = torch
+        eps_b = eps_bg if eps_b is None else eps_b
+        d = _PlanDesc()
+        d.period[:] = [float(p) for p in periods]
+        d.orders[:] = [int(n) for n in orders]
+        d.eps_bg_re, d.eps_bg_im = complex(eps_bg).real, complex(eps_bg).imag
+        d.eps_b_re, d.eps_b_im = complex(eps_b).real, complex(eps_b).imag
+        self._keep = []
+        if voxels is not None:
+            grid = np.ascontiguousarray(voxels, dtype=np.complex128)
+            d.voxels[:] = list(grid.shape)
+            d.eps_grid_host = grid.ctypes.data
+            d.n_shapes = 0
+            self._keep.append(grid)
+        else:
+            shapes = shapes or []
+            arr = (_Shape * max(len(shapes), 1))()
+            for i, s in enumerate(shapes):
+                arr[i].kind = int(s["kind"])
+                arr[i].center[:] = [float(v) for v in s["center"]]
+                arr[i].size[:] = [float(v) for v in s["size"]]
+                arr[i].eps_re, arr[i].eps_im = complex(s["eps"]).real, complex(s["eps"]).imag
+            d.n_shapes = len(shapes)
+            d.shapes = arr
+            d.voxels[:] = [0, 0, 0]
+            d.eps_grid_host = None
+            self._keep.append(arr)
+        d.max_iters, d.max_batch = int(max_iters), int(max_batch)
+        self.stream = stream
+        d.cuda_stream = stream.cuda_stream if stream is not None else None
+        self.orders = tuple(int(n) for n in orders)
+        self.n = int(np.prod(self.orders))
+        self.max_batch, self.max_iters = int(max_batch), int(max_iters)
+        h = C.c_void_p()
+        st = _lib.gsm_plan_create(C.byref(d), C.byref(h))
+        if st != OK:
+            raise GsmError(st, _lib.gsm_last_error(None).decode())
+        self._h = h
+
+    # -- lifetime -------------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.gsm_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- queries --------------------------------------------------------------------------------------------
+    def coeffs(self) -> np.ndarray:
+        N = self.orders
+        out = np.empty((2 * N[0] - 1, 2 * N[1] - 1, 2 * N[2] - 1), dtype=np.complex128)
+        _check(_lib.gsm_plan_coeffs(self._h, out.ctypes.data), self._h)
+        return out
+
+    def info(self):
+        g = (C.c_int * 3)()
+        b, l = C.c_longlong(), C.c_longlong()
+        _check(_lib.gsm_plan_info(self._h, g, C.byref(b), C.byref(l)), self._h)
+        return {"fft_grid": tuple(g), "device_bytes": b.value, "launches": l.value}
+
+    # -- hot path -------------------------------------------------------------------------------------------
+    def apply(self, k_bloch, k0, x, out=None):
+        """gsm_apply: y = x - G (T x).  x: cuda complex128 tensor [batch, 3, N1, N2, N3]; asynchronous."""
+        torch = self._torch
+        batch = x.shape[0]
+        assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous() and tuple(x.shape[1:]) == (3,) + self.orders
+        y = torch.empty_like(x) if out is None else out
+        kb, kk = _f64(k_bloch, (batch, 3)), _f64(k0, (batch,))
+        _check(_lib.gsm_apply(self._h, batch, kb.ctypes.data, kk.ctypes.data, x.data_ptr(), y.data_ptr()), self._h)
+        return y
+
+    def solve(self, k_bloch, k0, pol, tol=1e-10, out=None):
+        """gsm_solve: returns (E cuda tensor [3,N1,N2,N3], residual history, iterations, true residual, status)."""
+        torch = self._torch
+        E = torch.empty((3,) + self.orders, dtype=torch.complex128, device="cuda") if out is None else out
+        kb = _f64(k_bloch, (3,))
+        pl = _f64(np.asarray(pol, dtype=np.complex128).view(np.float64), (6,))
+        hist = np.zeros(self.max_iters)
+        it, res = C.c_int(), C.c_double()
+        st = _check(_lib.gsm_solve(self._h, kb.ctypes.data, float(k0), pl.ctypes.data, float(tol), E.data_ptr(),
+                                   hist.ctypes.data, self.max_iters, C.byref(it), C.byref(res)), self._h)
+        return E, hist[: it.value].copy(), it.value, res.value, st
+
+    def scan(self, k_bloch, k0, pol, tol=1e-10, fields=None):
+        """gsm_scan: returns (resp [npts,3] complex, iters [npts], resid [npts], status).
+
+        pol: [npts, 6] real (interleaved complex) or [npts, 3] complex.  fields: optional cuda tensor
+        [npts, 3, N1, N2, N3] that receives every solution."""
+        kb = _f64(k_bloch)
+        npts = kb.shape[0]
+        kk = _f64(k0, (npts,))
+        pl = np.asarray(pol)
+        if np.iscomplexobj(pl):
+            pl = np.ascontiguousarray(pl, dtype=np.complex128).view(np.float64)
+        pl = _f64(pl, (npts, 6))
+        resp = np.zeros((npts, 3), dtype=np.complex128)
+        iters = np.zeros(npts, dtype=np.int32)
+        resid = np.zeros(npts)
+        st = _check(_lib.gsm_scan(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol),
+                                  resp.ctypes.data, iters.ctypes.data, resid.ctypes.data,
+                                  fields.data_ptr() if fields is not None else None), self._h)
+        return resp, iters, resid, st
+
+
+def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):
+    """gsm_pole_search (host side): returns (eta [Np], zeta [Np], best index or -1)."""
+    kappa = _f64(kappa)
+    xi = np.ascontiguousarray(xi, dtype=np.complex128)
+    eta = np.zeros(Np, dtype=np.complex128)
+    zeta = np.zeros(Np, dtype=np.complex128)
+    best = C.c_int(-1)
+    lo = float(kappa[0]) if lo is None else float(lo)
+    hi = float(kappa[-1]) if hi is None else float(hi)
+    st = _lib.gsm_pole_search(len(kappa), kappa.ctypes.data, xi.ctypes.data, int(Np), int(Nd), lo, hi,
+                              eta.ctypes.data, zeta.ctypes.data, C.byref(best))
+    if st < 0:
+        raise GsmError(st, "gsm_pole_search: invalid arguments")
+    return eta, zeta, best.value
+
+
+def plan_from_geometry(geo, max_iters=64, max_batch=1, stream=None) -> Plan:
+    """Plan for a workloads.Geometry (seeded input description; holds no arithmetic of the method)."""
+    return Plan(geo.periods, geo.orders, shapes=geo.shapes, eps_bg=geo.eps_bg, eps_b=geo.eps_b, voxels=geo.voxels,
+                max_iters=max_iters, max_batch=max_batch, stream=stream)
