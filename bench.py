@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the GSM hot path on B200 (BASELINE.json metric: (k, omega) solves/s and operator applies/s
+at 31^3 orders; % of the HBM roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl gsm|reference]
+
+Workload (BASELINE.json config 5a; recipe in DESIGN.md "Input recipe"): random voxel composite
+(20 seeded spheres on a 128^3 voxel grid, cubic Lambda = 0.25 lambda), 31^3 Fourier orders (FFT grid 64^3), 256
+concurrent (k, omega) solves per GPU: kappa equidistant on n in [1.05, 1.20], k || z, a = x, GMRES tol 1e-10.
+One step = one pass of the whole hot path over that batch: gsm_scan of the 256 points (operator applies, Arnoldi /
+Gram-Schmidt, least squares, update, true residual, 0-th order response).  Inputs: the per-step working set is
+~24 GB of Krylov basis, far above the 126 MB L2, so no L2 flush is needed between timed iterations.
+
+Prints ONE JSON line (rank 0).  `value`: plan resident on the device (coefficient spectrum built).  `e2e`: per step
+the voxel grid is uploaded from pinned host memory and step a0 re-run (gsm_plan_set_cell), then the scan, the
+device->host read of the responses, and the host pole search.  `roofline`: dominant kernel class, timed live with CUDA
+events on the plan's stream inside the timed region (gsm_plan_profile).  `cpu_baseline`: the CPU oracle as it stands
+(O(n^2) Toeplitz product + full GMRES) on one of the 256 points.
+
+--impl reference: the oracle itself on the host cores, one solve (one point of the scan) per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "(k,omega) solves/s at 31^3 orders, batch 256"
+UNIT = "solves/s"
+ORDERS = (31, 31, 31)
+BATCH = 256
+TOL = 1e-10
+MAX_ITERS = 64
+N_LO, N_HI = 1.05, 1.20
+TWO_PI = 2.0 * np.pi
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _traffic(kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json)."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        return json.load(f).get(kernel, {}).get("dram_bytes_per_launch")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(rank, world):
+    """The scan list of this rank: BATCH points of a (BATCH * world)-point equidistant kappa mesh (weak scaling)."""
+    from paper_1501_01752_b200 import workloads as wl
+    geo = wl.voxel_composite(ORDERS, nv=128)
+    kappa_all = wl.kappa_mesh(N_LO, N_HI, BATCH * world)
+    kappa = kappa_all[rank * BATCH:(rank + 1) * BATCH]
+    kb, k0, pol = wl.scan_points(kappa, 2, 0)
+    return geo, kappa, kb, k0, pol
+
+
+def oracle_solve_once(geo, kb, k0, pol):
+    """One solve by the CPU oracle as it stands; returns (seconds, iterations, threads)."""
+    from oracle import gsm_oracle as orc
+    c = orc.coeffs_voxel(geo.voxels, geo.orders, geo.eps_b)
+    t0 = time.perf_counter()
+    _, hist, iters = orc.solve_gmres(c, geo.periods, geo.orders, kb, float(k0), geo.eps_b, pol[0::2] + 1j * pol[1::2],
+                                     tol=TOL, max_iters=MAX_ITERS, matvec=orc.toeplitz_matvec_c)
+    return time.perf_counter() - t0, iters, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from __graft_entry__ import build_oracle
+    build_oracle()
+    geo, kappa, kb, k0, pol = workload(0, 1)
+    times, its, cores = [], [], 1
+    for s in range(args.warmup + args.steps):
+        p = (s * 37) % BATCH
+        t, it, cores = oracle_solve_once(geo, kb[p], k0[p], pol[p])
+        if s >= args.warmup:
+            times.append(t); its.append(it)
+    total = float(np.sum(times))
+    value = len(times) / total
+    sample = f"1 of the {BATCH} (k,omega) points per step (full GMRES solve, O(n^2) Toeplitz product), mean {np.mean(its):.1f} iterations"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAME, "orders": list(ORDERS), "batch": 1, "tol": TOL},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+WORKLOAD_NAME = ("config5a: random voxel composite (20 seeded spheres, 128^3 voxels, Lambda=0.25 lambda), 31^3 orders, "
+                 "FFT grid 64^3, 256 concurrent (k,omega) solves per GPU, complex fp64, GMRES tol 1e-10")
+
+
+def run_gsm(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the GSM hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import __graft_entry__ as ge
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        dist.barrier()
+    from paper_1501_01752_b200 import gsm
+
+    geo, kappa, kb, k0, pol = workload(rank, world)
+    stream = torch.cuda.Stream()
+    plan = gsm.plan_from_geometry(geo, max_iters=MAX_ITERS, max_batch=BATCH, stream=stream)
+    pinned_grid = torch.from_numpy(geo.voxels).pin_memory()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def step():
+        return plan.scan(kb, k0, pol, tol=TOL)
+
+    def step_e2e():
+        plan.set_cell(geo.periods, eps_bg=geo.eps_bg, eps_b=geo.eps_b, voxels=pinned_grid)
+        resp, iters, resid, st = plan.scan(kb, k0, pol, tol=TOL)
+        eta, zeta, best = gsm.pole_search(kappa, resp[:, 0], 5, 10)
+        return resp, iters, resid, st, (eta[best] if best >= 0 else None)
+
+    for _ in range(args.warmup):
+        resp, iters, resid, st = step()
+    assert st >= 0 and float(np.max(resid)) <= 1e-9, f"solve failed: status {st}, max residual {np.max(resid):.2e}"
+
+    # ---- device-resident timed region --------------------------------------------------------------------------
+    sampler = ClockSampler(local)
+    plan.profile(True)
+    plan.profile_read(reset=True)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        resp, iters, resid, st = step()
+    e1.record(stream)
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop() if rank == 0 else None
+    prof = plan.profile_read(reset=True)
+    plan.profile(False)
+    value = BATCH * world * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers ---------------------------------------------------------
+    for _ in range(min(args.warmup, 2)):
+        step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        out = step_e2e()
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e_value = BATCH * world * args.steps / e2e_s
+    h2d = int(pinned_grid.numel() * 16 + kb.nbytes + k0.nbytes + pol.nbytes + 16)
+    d2h = int(resp.nbytes + iters.nbytes + resid.nbytes + 4 * int(np.max(iters)))   # + nactive read per iteration
+
+    # ---- operator applies/s (the other half of BASELINE.json's metric) -------------------------------------------
+    x = torch.randn((BATCH, 3) + ORDERS, dtype=torch.complex128, device="cuda")
+    y = torch.empty_like(x)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        plan.apply(kb, k0, x, out=y)
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    napply = 20
+    barrier()
+    a0.record(stream)
+    for _ in range(napply):
+        plan.apply(kb, k0, x, out=y)
+    a1.record(stream)
+    barrier()
+    apply_ms = max_over_ranks(a0.elapsed_time(a1)) / napply
+    V = 16.0 * 3 * geo.n
+    chat_bytes = 16.0 * 64 ** 3
+    apply_alg_bytes = 2 * V * BATCH + chat_bytes
+
+    if world > 1:
+        dist.barrier()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel class -----------------------------------------------------------------
+    peak, peak_src = _peaks()
+    timed = {k: v for k, v in prof.items() if v[0] > 0 and k != "plan"}
+    dom = max(timed, key=lambda k: timed[k][1])
+    n_l, ms_l, by_l = timed[dom]
+    achieved = by_l / (ms_l * 1e-3) / 1e9
+    kernels_ms = sum(v[1] for v in timed.values())
+    gpu_launches = int(sum(v[0] for v in timed.values()))
+    mean_it = float(np.mean(iters))
+    # whole-step figure against SURVEY 8(d)'s B_solve = (m(m+1)/2 + 3m + 1) V + m |Chat| per solve
+    b_solve = float(np.sum((iters * (iters + 1.0) / 2 + 3.0 * iters + 1.0) * V)) + float(np.max(iters)) * chat_bytes
+    path_gbs = b_solve * args.steps / (ms_total * 1e-3) / 1e9
+
+    # ---- CPU oracle on a bounded sample ---------------------------------------------------------------------------
+    cpu_t, cpu_it, cores = oracle_solve_once(geo, kb[0], k0[0], pol[0])
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_NAME, "orders": list(ORDERS), "fft_grid": list(plan.info()["fft_grid"]),
+                   "batch_per_gpu": BATCH, "tol": TOL, "max_iters": MAX_ITERS, "mean_iters": mean_it,
+                   "max_true_resid": float(np.max(resid)), "parallelism": f"scan list sharded over {world} GPU(s), no collective",
+                   "l2": "working set per step ~24 GB >> 126 MB L2; no flush needed"},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "includes": "voxel grid H2D from pinned memory + a0 (gsm_plan_set_cell) + gsm_scan + response D2H + host pole search"},
+        "gpu_launches": gpu_launches,
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": _traffic(dom), "peak_source": peak_src,
+                     "launches": n_l, "avg_launch_ms": ms_l / n_l, "algorithmic_bytes_per_launch": by_l / n_l,
+                     "share_of_step": ms_l / kernels_ms},
+        "path_roofline": {"algorithmic_GBps": path_gbs, "frac": path_gbs / peak,
+                          "definition": "SURVEY 8(d) B_solve summed over the batch / step time"},
+        "kernel_ms_per_step": {k: v[1] / args.steps for k, v in timed.items()},
+        "kernel_GBps": {k: (v[2] / (v[1] * 1e-3) / 1e9 if v[1] > 0 and v[2] > 0 else None) for k, v in timed.items()},
+        "applies_per_s": BATCH * world / (apply_ms * 1e-3),
+        "apply": {"ms_per_batch_apply": apply_ms, "algorithmic_GBps": apply_alg_bytes / (apply_ms * 1e-3) / 1e9,
+                  "frac": apply_alg_bytes / (apply_ms * 1e-3) / 1e9 / peak, "definition": "(2V x 256 + |Chat|) / time"},
+        "cpu_baseline": {"value": 1.0 / cpu_t, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"1 of the {BATCH} (k,omega) points (full GMRES solve with the O(n^2) Toeplitz product, "
+                                   f"{cpu_it} iterations, {cpu_t:.1f} s)"},
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="gsm", choices=["gsm", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gsm(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -89,6 +89,23 @@ gsm_status gsm_plan_coeffs(const gsm_plan* plan, double* host_out);
 /* FFT grid sizes P1..P3 chosen by the plan, device bytes held, and the number of kernel launches enqueued so far. */
 gsm_status gsm_plan_info(const gsm_plan* plan, int fft_grid[3], long long* device_bytes, long long* launches);
 
+/* Replace the cell of an existing plan - periods, permittivities and shapes or voxel grid, i.e. step a0 (PAPER.md:62,
+ * :99: the harmonics depend only on the geometry) - keeping orders, max_iters, max_batch and every workspace.
+ * desc->orders must equal the plan's; voxel grids follow the rules of gsm_plan_create.  Host arrays in desc are read
+ * before return and not retained. */
+gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* desc);
+
+/* Launch accounting.  Every kernel the library enqueues is counted per kernel class (gsm_kernel_class_count()
+ * classes, names from gsm_kernel_class_name(cls)).  gsm_plan_profile(plan, 1) additionally brackets every launch
+ * with a CUDA event pair on the plan's stream; gsm_plan_profile_read synchronises the stream and returns, for the
+ * first ncls classes, the launch counts, the summed device time in milliseconds and the summed algorithmic bytes
+ * (the minimal reads + writes of each launch as designed) since the last reset (any array may
+ * be NULL); reset != 0 clears them.  Times are zero for launches made while profiling was off. */
+gsm_status gsm_plan_profile(gsm_plan* plan, int enable);
+gsm_status gsm_plan_profile_read(gsm_plan* plan, int ncls, long long* launches, double* ms, double* bytes, int reset);
+int gsm_kernel_class_count(void);
+const char* gsm_kernel_class_name(int cls);
+
 /* Operator apply, Eq. 4 left-hand side: y[b] = x[b] - G(k_bloch[b], k0[b]) (T x[b]), b < batch.
  * k_bloch[batch][3], k0[batch] are host arrays (copied before return).  d_x, d_y: device, [batch][3][N1][N2][N3]
  * complex; they must not overlap.  1 <= batch <= max_batch.  Asynchronous on the plan's stream. */

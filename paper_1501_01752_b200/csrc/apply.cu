@@ -170,12 +170,17 @@ size_t apply_smem_max(const ApplyGeom& g) {
 }
 
 cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
-                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, long long* launches) {
+                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact) {
     const int nlt = (g.NL + g.L - 1) / g.L;
-    z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active);
-    xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active);
-    z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active);
-    if (launches) *launches += 3;
+    // algorithmic bytes of the three passes as designed: field vector V = 3n, z-transformed intermediate 3 P3 NL
+    const double V = 16.0 * 3.0 * g.n * nact, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL * nact;
+    const double Cb = 16.0 * g.ax[0].P * g.ax[1].P * g.ax[2].P;
+    { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
+      z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active); }
+    { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
+      xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); }
+    { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
+      z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); }
     return cudaGetLastError();
 }
 

@@ -20,8 +20,14 @@ struct gsm_plan {
     int max_batch = 1, max_iters = 64;
     long i0 = 0;                  // flat index of m = 0 inside one component
     std::vector<void*> allocs;    // every device allocation, freed in destroy
-    long long device_bytes = 0, launches = 0;
-    cplx *coef = nullptr, *chat = nullptr, *W = nullptr, *xbuf = nullptr, *ybuf = nullptr;
+    long long device_bytes = 0;
+    Profiler prof;
+    cplx *coef = nullptr, *chat = nullptr, *pad = nullptr, *W = nullptr, *xbuf = nullptr, *ybuf = nullptr;
+    size_t vgrid_count = 0;
+    cplx* vgrid = nullptr;        // voxel path: device copy of the grid, transformed in place
+    const cplx* vtw[3] = {nullptr, nullptr, nullptr};
+    int* vpos[3] = {nullptr, nullptr, nullptr};
+    int vdim[3] = {0, 0, 0};
     double *d_kvec = nullptr, *d_k0 = nullptr, *d_resid = nullptr;
     void* pinned = nullptr;       // host staging: nactive, iters, resid, hist
     size_t pinned_bytes = 0;
@@ -124,7 +130,7 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     const gsm_plan_desc& d = plan->desc;
     const int* N = d.orders;
     const size_t ncoef = (size_t)(2 * N[0] - 1) * (2 * N[1] - 1) * (2 * N[2] - 1);
-    CK(dalloc(plan, &plan->coef, ncoef));
+    if (!plan->coef) CK(dalloc(plan, &plan->coef, ncoef));
     if (d.eps_grid_host == nullptr) {
         std::vector<ShapeDev> hs(std::max(d.n_shapes, 1));
         const double vol = d.period[0] * d.period[1] * d.period[2];
@@ -144,7 +150,10 @@ static gsm_status build_coeffs(gsm_plan* plan) {
         CK(cudaMalloc(&dsh, sizeof(ShapeDev) * hs.size()));
         cudaError_t e = cudaMemcpyAsync(dsh, hs.data(), sizeof(ShapeDev) * hs.size(), cudaMemcpyHostToDevice, plan->stream);
         const cplx c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_b_re, d.eps_b_im);
-        if (e == cudaSuccess) e = launch_coeffs_analytic(dsh, d.n_shapes, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
+        if (e == cudaSuccess) {
+            ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
+            e = launch_coeffs_analytic(dsh, d.n_shapes, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
+        }
         if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
         cudaFree(dsh);
         CK(e);
@@ -153,28 +162,31 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     // voxel path: forward FFT of (eps - eps_b)/eps_b on the Nv grid, keep |d_a| <= N_a - 1
     const int* V = d.voxels;
     AxisPlan vax[3];
-    const cplx* vtw[3];
-    int* dpos[3] = {nullptr, nullptr, nullptr};
-    for (int a = 0; a < 3; ++a) {
+    for (int a = 0; a < 3; ++a)
         if (V[a] < 2 * N[a] - 1 || V[a] > 512 || !make_axis(V[a], V[a], &vax[a]))
             return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
-        CK(upload_twiddles(plan, V[a], &vtw[a]));
-        std::vector<int> pos(V[a]);
-        for (int k = 0; k < V[a]; ++k) pos[k] = pos_of_freq(k, V[a], vax[a].radix, vax[a].nst);
-        CK(dalloc(plan, &dpos[a], (size_t)V[a]));
-        CK(cudaMemcpy(dpos[a], pos.data(), sizeof(int) * V[a], cudaMemcpyHostToDevice));
+    if (!plan->vtw[0] || plan->vdim[0] != V[0] || plan->vdim[1] != V[1] || plan->vdim[2] != V[2]) {
+        for (int a = 0; a < 3; ++a) {   // twiddles and frequency->position tables of the voxel FFT (kept for re-use)
+            CK(upload_twiddles(plan, V[a], &plan->vtw[a]));
+            std::vector<int> pos(V[a]);
+            for (int k = 0; k < V[a]; ++k) pos[k] = pos_of_freq(k, V[a], vax[a].radix, vax[a].nst);
+            CK(dalloc(plan, &plan->vpos[a], (size_t)V[a]));
+            CK(cudaMemcpy(plan->vpos[a], pos.data(), sizeof(int) * V[a], cudaMemcpyHostToDevice));
+            plan->vdim[a] = V[a];
+        }
     }
+    const cplx* const* vtw = plan->vtw;
+    int* const* dpos = plan->vpos;
     const size_t nv = (size_t)V[0] * V[1] * V[2];
-    cplx* grid = nullptr;
-    CK(cudaMalloc(&grid, sizeof(cplx) * nv));
+    if (!plan->vgrid || plan->vgrid_count != nv) { CK(dalloc(plan, &plan->vgrid, nv)); plan->vgrid_count = nv; }
+    cplx* grid = plan->vgrid;
     cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
+    ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
     if (e == cudaSuccess) e = launch_voxel_prepare(grid, (long)nv, d.eps_b_re, d.eps_b_im, plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0] * V[1], vax[2], 1, vtw[2], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0], vax[1], V[2], vtw[1], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, 1, vax[0], (long)V[1] * V[2], vtw[0], plan->stream);
     if (e == cudaSuccess) e = launch_voxel_extract(grid, V, N, dpos[0], dpos[1], dpos[2], plan->coef, plan->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
-    cudaFree(grid);
     CK(e);
     return GSM_OK;
 }
@@ -185,17 +197,16 @@ static gsm_status build_spectrum(gsm_plan* plan) {
     const int P[3] = {g.ax[0].P, g.ax[1].P, g.ax[2].P};
     const int N[3] = {g.N1, g.N2, g.N3};
     const size_t np = (size_t)P[0] * P[1] * P[2];
-    CK(dalloc(plan, &plan->chat, np));
-    cplx* pad = nullptr;
-    CK(cudaMalloc(&pad, sizeof(cplx) * np));
+    if (!plan->chat) CK(dalloc(plan, &plan->chat, np));
+    if (!plan->pad) CK(dalloc(plan, &plan->pad, np));
+    cplx* pad = plan->pad;
+    ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
     cudaError_t e = launch_embed(plan->coef, N, P, pad, plan->stream);
     AxisPlan full[3] = {g.ax[0], g.ax[1], g.ax[2]};
     if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0] * P[1], full[2], 1, g.tw[2], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0], full[1], P[2], g.tw[1], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(pad, 1, full[0], (long)P[1] * P[2], g.tw[0], plan->stream);
     if (e == cudaSuccess) e = launch_chat_layout(pad, P, plan->chat, plan->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
-    cudaFree(pad);
     CK(e);
     g.chat = plan->chat;
     return GSM_OK;
@@ -246,6 +257,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         if (s2 != GSM_OK) return s2;
         s2 = build_spectrum(plan);
         if (s2 != GSM_OK) return s2;
+        CK(cudaStreamSynchronize(plan->stream));
         // workspaces
         const int B = plan->max_batch, m = plan->max_iters;
         KrylovDims& kd = plan->kd;
@@ -295,6 +307,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
 extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
     if (!plan) return GSM_E_INVALID;
     cudaStreamSynchronize(plan->stream);
+    plan->prof.destroy();
     for (void* p : plan->allocs) cudaFree(p);
     if (plan->pinned) cudaFreeHost(plan->pinned);
     delete plan;
@@ -314,7 +327,10 @@ extern "C" gsm_status gsm_plan_info(const gsm_plan* plan, int fft_grid[3], long 
     if (!plan) return GSM_E_INVALID;
     if (fft_grid) for (int a = 0; a < 3; ++a) fft_grid[a] = plan->geom.ax[a].P;
     if (device_bytes) *device_bytes = plan->device_bytes;
-    if (launches) *launches = plan->launches;
+    if (launches) {
+        *launches = 0;
+        for (int c = 0; c < KC_COUNT; ++c) *launches += plan->prof.launches[c];
+    }
     return GSM_OK;
 }
 
@@ -360,7 +376,7 @@ extern "C" gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch
     CK(cudaMemcpyAsync(plan->d_kvec, k_bloch, sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, plan->stream));
     CK(cudaMemcpyAsync(plan->d_k0, k0, sizeof(double) * batch, cudaMemcpyHostToDevice, plan->stream));
     CK(launch_apply(plan->geom, batch, plan->d_kvec, plan->d_k0, static_cast<const cplx*>(d_x), static_cast<cplx*>(d_y),
-                    plan->W, nullptr, plan->stream, &plan->launches));
+                    plan->W, nullptr, plan->stream, &plan->prof, batch));
     return GSM_OK;
 }
 
@@ -381,29 +397,28 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     CK(cudaMemcpyAsync(ks.tol, &tol, sizeof(double), cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ks.nactive, &nb, sizeof(int), cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(ks.basis, 0, sizeof(cplx) * (size_t)nb * kd.vlen, st));
-    CK(launch_krylov_init(kd, ks, nb, plan->i0, g.n, st));
-    plan->launches += 1;
+    Profiler* prof = &plan->prof;
+    CK(launch_krylov_init(kd, ks, nb, plan->i0, g.n, st, prof));
     const size_t vs = (size_t)nb * kd.vlen;
-    int j = 0;
+    int j = 0, nact = nb;   // nact: solves still iterating (read back once per iteration)
     for (; j < kd.mmax; ++j) {
         CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
-                        plan->W, ks.active, st, &plan->launches));
-        CK(launch_sweep_dots(kd, ks, nb, j, st));
-        CK(launch_hsolve(kd, ks, nb, j, st));
-        CK(launch_sweep_update(kd, ks, nb, j, st));
-        CK(launch_givens(kd, ks, nb, j, st));
-        CK(launch_normalize(kd, ks, nb, j, st));
-        plan->launches += 5;
+                        plan->W, ks.active, st, prof, nact));
+        CK(launch_sweep_dots(kd, ks, nb, j, st, prof, nact));
+        CK(launch_hsolve(kd, ks, nb, j, st, prof));
+        CK(launch_sweep_update(kd, ks, nb, j, st, prof, nact));
+        CK(launch_givens(kd, ks, nb, j, st, prof));
+        CK(launch_normalize(kd, ks, nb, j, st, prof, nact));
         CK(cudaMemcpyAsync(pin_i, ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-        if (pin_i[0] <= 0) break;
+        nact = pin_i[0];
+        if (nact <= 0) break;
     }
-    CK(launch_backsolve(kd, ks, nb, st));
-    CK(launch_combine(kd, ks, nb, d_E, st));
+    CK(launch_backsolve(kd, ks, nb, st, prof));
+    CK(launch_combine(kd, ks, nb, d_E, st, prof));
     // true residual with one more apply
-    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, nullptr, st, &plan->launches));
-    CK(launch_true_residual(kd, ks, nb, plan->ybuf, plan->i0, g.n, plan->d_resid, st));
-    plan->launches += 4;
+    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, nullptr, st, prof, nb));
+    CK(launch_true_residual(kd, ks, nb, plan->ybuf, plan->i0, g.n, plan->d_resid, st, prof));
     int* h_iters = reinterpret_cast<int*>(pin + 2);
     double* h_resid = pin + 2 + nb;           // ints occupy at most nb doubles
     int* h_active = reinterpret_cast<int*>(pin + 2 + 2 * (size_t)nb);
@@ -457,4 +472,115 @@ extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, 
         if (s != GSM_OK) return s;
     }
     return nc ? GSM_NOT_CONVERGED : GSM_OK;
+}
+
+
+// ---- profiler (gsm_plan_profile / gsm_plan_profile_read) ---------------------------------------------------------
+namespace gsm {
+static const char* const kKernelClassNames[KC_COUNT] = {
+    "z_forward", "xy_conv", "z_inverse_green", "sweep_dots", "hsolve", "sweep_update", "givens", "normalize",
+    "combine", "residual", "small", "plan"};
+const char* kernel_class_name(int cls) { return cls >= 0 && cls < KC_COUNT ? kKernelClassNames[cls] : ""; }
+
+void Profiler::begin(int c, cudaStream_t st, double nbytes) {
+    launches[c] += 1;
+    bytes[c] += nbytes;
+    if (!on) return;
+    if (2 * used + 1 >= ev.size()) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { on = false; return; }
+        ev.push_back(a);
+        ev.push_back(b);
+        cls.push_back(c);
+    }
+    cls[used] = c;
+    cudaEventRecord(ev[2 * used], st);
+}
+void Profiler::end(cudaStream_t st) {
+    if (!on) return;
+    cudaEventRecord(ev[2 * used + 1], st);
+    ++used;
+}
+cudaError_t Profiler::collect() {
+    for (size_t i = 0; i < used; ++i) {
+        cudaError_t e = cudaEventSynchronize(ev[2 * i + 1]);
+        if (e != cudaSuccess) return e;
+        float t = 0.f;
+        e = cudaEventElapsedTime(&t, ev[2 * i], ev[2 * i + 1]);
+        if (e != cudaSuccess) return e;
+        ms[cls[i]] += (double)t;
+    }
+    used = 0;
+    return cudaSuccess;
+}
+void Profiler::reset() {
+    used = 0;
+    for (int c = 0; c < KC_COUNT; ++c) { launches[c] = 0; ms[c] = 0.0; bytes[c] = 0.0; }
+}
+void Profiler::destroy() {
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    ev.clear();
+    cls.clear();
+    used = 0;
+}
+}  // namespace gsm
+
+extern "C" gsm_status gsm_plan_profile(gsm_plan* plan, int enable) {
+    if (!plan) return GSM_E_INVALID;
+    CK(cudaStreamSynchronize(plan->stream));
+    CK(plan->prof.collect());
+    plan->prof.on = enable != 0;
+    return GSM_OK;
+}
+
+extern "C" int gsm_kernel_class_count(void) { return KC_COUNT; }
+extern "C" const char* gsm_kernel_class_name(int cls) { return kernel_class_name(cls); }
+
+extern "C" gsm_status gsm_plan_profile_read(gsm_plan* plan, int ncls, long long* launches, double* ms, double* bytes,
+                                            int reset) {
+    if (!plan || ncls < 0) return GSM_E_INVALID;
+    CK(cudaStreamSynchronize(plan->stream));
+    CK(plan->prof.collect());
+    for (int c = 0; c < ncls && c < KC_COUNT; ++c) {
+        if (launches) launches[c] = plan->prof.launches[c];
+        if (ms) ms[c] = plan->prof.ms[c];
+        if (bytes) bytes[c] = plan->prof.bytes[c];
+    }
+    if (reset) plan->prof.reset();
+    return GSM_OK;
+}
+
+// Replace the cell (shapes or voxel grid, permittivities, periods) of an existing plan without reallocating the
+// workspaces: re-runs step a0 (coefficients and their spectrum).  orders must be unchanged.
+extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* desc) {
+    if (!plan) return GSM_E_INVALID;
+    if (!desc) return fail(plan, GSM_E_INVALID, "gsm_plan_set_cell: null descriptor");
+    for (int a = 0; a < 3; ++a) {
+        if (desc->orders[a] != plan->desc.orders[a]) return fail(plan, GSM_E_INVALID, "gsm_plan_set_cell: orders differ");
+        if (!(desc->period[a] > 0.0)) return fail(plan, GSM_E_INVALID, "periods must be positive");
+    }
+    if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(plan, GSM_E_INVALID, "eps_b must be non-zero");
+    if (desc->eps_grid_host == nullptr && (desc->n_shapes < 0 || (desc->n_shapes > 0 && !desc->shapes)))
+        return fail(plan, GSM_E_INVALID, "shapes missing");
+    const gsm_plan_desc old = plan->desc;
+    plan->desc.eps_bg_re = desc->eps_bg_re; plan->desc.eps_bg_im = desc->eps_bg_im;
+    plan->desc.eps_b_re = desc->eps_b_re;   plan->desc.eps_b_im = desc->eps_b_im;
+    plan->desc.n_shapes = desc->n_shapes;   plan->desc.shapes = desc->shapes;
+    plan->desc.eps_grid_host = desc->eps_grid_host;
+    for (int a = 0; a < 3; ++a) {
+        plan->desc.period[a] = desc->period[a];
+        plan->desc.voxels[a] = desc->voxels[a];
+        plan->geom.K[a] = 2.0 * M_PI / desc->period[a];
+    }
+    plan->geom.epsb_re = desc->eps_b_re; plan->geom.epsb_im = desc->eps_b_im;
+    gsm_status s = build_coeffs(plan);
+    if (s == GSM_OK) s = build_spectrum(plan);
+    if (s == GSM_OK) {
+        cudaError_t e = cudaStreamSynchronize(plan->stream);
+        if (e != cudaSuccess) s = fail(plan, GSM_E_CUDA, cudaGetErrorString(e));
+    }
+    plan->desc.shapes = nullptr;          // caller-owned arrays are not retained
+    plan->desc.eps_grid_host = nullptr;
+    (void)old;
+    return s;
 }

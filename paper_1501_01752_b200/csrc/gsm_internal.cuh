@@ -9,6 +9,35 @@
 
 namespace gsm {
 
+// Kernel classes for launch counting and (optional) per-class CUDA-event timing (gsm_plan_profile).
+enum KernelClass {
+    KC_Z_FORWARD = 0, KC_XY_CONV, KC_Z_INVERSE_GREEN, KC_SWEEP_DOTS, KC_HSOLVE, KC_SWEEP_UPDATE, KC_GIVENS,
+    KC_NORMALIZE, KC_COMBINE, KC_RESIDUAL, KC_SMALL, KC_PLAN, KC_COUNT
+};
+const char* kernel_class_name(int cls);
+
+// Counts every kernel launch per class; when `on`, also brackets each launch with a CUDA event pair on the launch
+// stream (events are pooled and read back by collect()).
+struct Profiler {
+    bool on = false;
+    long long launches[KC_COUNT] = {};
+    double ms[KC_COUNT] = {};
+    double bytes[KC_COUNT] = {};   // algorithmic bytes (minimal reads + writes of that kernel), summed over launches
+    std::vector<cudaEvent_t> ev;   // pairs: ev[2i] start, ev[2i+1] stop
+    std::vector<int> cls;
+    size_t used = 0;
+    void begin(int c, cudaStream_t st, double nbytes);
+    void end(cudaStream_t st);
+    cudaError_t collect();          // sync the events recorded so far and add their durations to ms[]
+    void reset();
+    void destroy();
+};
+struct ProfScope {
+    Profiler* p; cudaStream_t st;
+    ProfScope(Profiler* p_, int c, cudaStream_t st_, double nbytes = 0.0) : p(p_), st(st_) { if (p) p->begin(c, st, nbytes); }
+    ~ProfScope() { if (p) p->end(st); }
+};
+
 // Geometry of the operator apply shared by the three passes.
 struct ApplyGeom {
     AxisPlan ax[3];      // x, y, z axes of the circulant grid
@@ -39,7 +68,7 @@ struct KrylovDims {
 // y[b] = x[b] - G_b (T x[b]); kvec[b][3], k0[b] device arrays; W workspace [batch][3][P3][NL].
 // active (may be null): per-solve flags; CTAs of solves with active[b] == 0 exit at once.
 cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
-                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, long long* launches);
+                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact);
 size_t apply_smem_max(const ApplyGeom& g);
 cudaError_t apply_init_attributes();
 cudaError_t plan_init_attributes();
@@ -81,17 +110,17 @@ struct KrylovState {   // all device pointers, one entry (or row) per solve of t
     double* tol;       // [1]
 };
 cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0 /*index of m=0*/, long n,
-                               cudaStream_t st);
-cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
-cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
-cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
-cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
-cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st);
-cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st);
-cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st);
+                               cudaStream_t st, Profiler* prof);
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st, Profiler* prof);
 // resid[b] = || pol delta_m0 - y[b] || / beta[b]
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
-                                 double* d_resid, cudaStream_t st);
+                                 double* d_resid, cudaStream_t st, Profiler* prof);
 cudaError_t krylov_init_attributes();
 
 }  // namespace gsm

@@ -333,42 +333,52 @@ cudaError_t krylov_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(sweep_dots_kernel<GSM_E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
     return e;
 }
-cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st) {
+cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
     krylov_init_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, i0, n);
     return cudaGetLastError();
 }
-cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
+    ProfScope ps_(prof, KC_SWEEP_DOTS, st, 16.0 * d.vlen * (j + 2.0) * nact);   // reads w and v_0..v_j
     const size_t smem = sizeof(double) * 4 * (KT / 32) * (size_t)(j + 1);
     sweep_dots_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, smem, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_HSOLVE, st);
     hsolve_kernel<<<batch, 32, sizeof(cplx) * d.ld, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
+    ProfScope ps_(prof, KC_SWEEP_UPDATE, st, 16.0 * d.vlen * (j + 3.0) * nact);   // reads w, v_0..v_j; writes w
     sweep_update_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * (j + 1), st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_GIVENS, st);
     givens_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st) {
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
+    ProfScope ps_(prof, KC_NORMALIZE, st, 16.0 * d.vlen * 2.0 * nact);
     normalize_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st) {
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
     backsolve_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch);
     return cudaGetLastError();
 }
-cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st) {
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_COMBINE, st, 16.0 * d.vlen * batch * (d.mmax / 2 + 1.0));
     combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_E);
     return cudaGetLastError();
 }
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
-                                 double* d_resid, cudaStream_t st) {
-    resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, d_y, i0, n);
+                                 double* d_resid, cudaStream_t st, Profiler* prof) {
+    { ProfScope ps_(prof, KC_RESIDUAL, st);
+    resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, d_y, i0, n); }
+    ProfScope ps2_(prof, KC_SMALL, st);
     resid_final_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, d_resid);
     return cudaGetLastError();
 }

@@ -55,10 +55,17 @@ def _load():
     lib.gsm_solve.argtypes = [P, P, C.c_double, P, C.c_double, P, P, C.c_int, ip, dp]
     lib.gsm_scan.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P]
     lib.gsm_pole_search.argtypes = [C.c_int, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P, ip]
+    lib.gsm_plan_set_cell.argtypes = [P, C.POINTER(_PlanDesc)]
+    lib.gsm_plan_profile.argtypes = [P, C.c_int]
+    lib.gsm_plan_profile_read.argtypes = [P, C.c_int, C.POINTER(C.c_longlong), dp, dp, C.c_int]
+    lib.gsm_kernel_class_count.argtypes = []
+    lib.gsm_kernel_class_count.restype = C.c_int
+    lib.gsm_kernel_class_name.argtypes = [C.c_int]
+    lib.gsm_kernel_class_name.restype = C.c_char_p
     lib.gsm_last_error.argtypes = [P]
     lib.gsm_last_error.restype = C.c_char_p
     for f in ("gsm_plan_create", "gsm_plan_destroy", "gsm_plan_coeffs", "gsm_plan_info", "gsm_apply", "gsm_solve",
-              "gsm_scan", "gsm_pole_search"):
+              "gsm_scan", "gsm_pole_search", "gsm_plan_set_cell", "gsm_plan_profile", "gsm_plan_profile_read"):
         getattr(lib, f).restype = C.c_int
     return lib
 
@@ -89,19 +96,37 @@ class Plan:
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1501_01752_b200.gsm needs a CUDA device; there is no CPU fallback")
         self._torch = torch
+        self.stream = stream
+        self.orders = tuple(int(n) for n in orders)
+        d, keep = self._desc(periods, shapes, eps_bg, eps_b, voxels, max_iters, max_batch)
+        self.n = int(np.prod(self.orders))
+        self.max_batch, self.max_iters = int(max_batch), int(max_iters)
+        self._keep = [keep]
+        h = C.c_void_p()
+        st = _lib.gsm_plan_create(C.byref(d), C.byref(h))
+        if st != OK:
+            raise GsmError(st, _lib.gsm_last_error(None).decode())
+        self._h = h
+
+    def _desc(self, periods, shapes, eps_bg, eps_b, voxels, max_iters, max_batch):
+        """Marshal a gsm_plan_desc; `voxels` may be a complex128 numpy array or a (pinned) CPU torch tensor."""
         eps_b = eps_bg if eps_b is None else eps_b
         d = _PlanDesc()
         d.period[:] = [float(p) for p in periods]
-        d.orders[:] = [int(n) for n in orders]
+        d.orders[:] = list(self.orders)
         d.eps_bg_re, d.eps_bg_im = complex(eps_bg).real, complex(eps_bg).imag
         d.eps_b_re, d.eps_b_im = complex(eps_b).real, complex(eps_b).imag
-        self._keep = []
         if voxels is not None:
-            grid = np.ascontiguousarray(voxels, dtype=np.complex128)
+            if hasattr(voxels, "data_ptr"):          # torch CPU tensor (e.g. pinned), complex128, contiguous
+                assert not voxels.is_cuda and voxels.is_contiguous() and voxels.dtype == self._torch.complex128
+                grid, ptr = voxels, voxels.data_ptr()
+            else:
+                grid = np.ascontiguousarray(voxels, dtype=np.complex128)
+                ptr = grid.ctypes.data
             d.voxels[:] = list(grid.shape)
-            d.eps_grid_host = grid.ctypes.data
+            d.eps_grid_host = ptr
             d.n_shapes = 0
-            self._keep.append(grid)
+            keep = grid
         else:
             shapes = shapes or []
             arr = (_Shape * max(len(shapes), 1))()
@@ -114,18 +139,29 @@ class Plan:
             d.shapes = arr
             d.voxels[:] = [0, 0, 0]
             d.eps_grid_host = None
-            self._keep.append(arr)
+            keep = arr
         d.max_iters, d.max_batch = int(max_iters), int(max_batch)
-        self.stream = stream
-        d.cuda_stream = stream.cuda_stream if stream is not None else None
-        self.orders = tuple(int(n) for n in orders)
-        self.n = int(np.prod(self.orders))
-        self.max_batch, self.max_iters = int(max_batch), int(max_iters)
-        h = C.c_void_p()
-        st = _lib.gsm_plan_create(C.byref(d), C.byref(h))
-        if st != OK:
-            raise GsmError(st, _lib.gsm_last_error(None).decode())
-        self._h = h
+        d.cuda_stream = self.stream.cuda_stream if self.stream is not None else None
+        return d, keep
+
+    def set_cell(self, periods, shapes=None, eps_bg=1.0, eps_b=None, voxels=None):
+        """gsm_plan_set_cell: re-run step a0 for a new cell with the same orders, keeping all workspaces."""
+        d, keep = self._desc(periods, shapes, eps_bg, eps_b, voxels, self.max_iters, self.max_batch)
+        _check(_lib.gsm_plan_set_cell(self._h, C.byref(d)), self._h)
+        del keep
+
+    def profile(self, enable=True):
+        """gsm_plan_profile: bracket every kernel launch with CUDA events on the plan's stream."""
+        _check(_lib.gsm_plan_profile(self._h, 1 if enable else 0), self._h)
+
+    def profile_read(self, reset=False):
+        """gsm_plan_profile_read: {class name: (launches, total ms, algorithmic bytes)}."""
+        n = _lib.gsm_kernel_class_count()
+        cnt = (C.c_longlong * n)()
+        ms = (C.c_double * n)()
+        by = (C.c_double * n)()
+        _check(_lib.gsm_plan_profile_read(self._h, n, cnt, ms, by, 1 if reset else 0), self._h)
+        return {_lib.gsm_kernel_class_name(c).decode(): (int(cnt[c]), float(ms[c]), float(by[c])) for c in range(n)}
 
     # -- lifetime -------------------------------------------------------------------------------------------
     def close(self):
