@@ -1,0 +1,254 @@
+// arnoldi_cluster.cu - one Arnoldi step of GMRES with literal modified Gram-Schmidt ("GMRes ...
+// according to Saad with the modified Gram-Schmidt orthogonalization"), each basis vector read from HBM ONCE.
+//
+//   for i = 0..j:  h_i = <v_i, w>;  w <- w - h_i v_i          (Saad Alg. 6.9, lines 4-7)
+//   h_{j+1,j} = ||w||;  v_{j+1} = w / h_{j+1,j}               (lines 8-9), then the Givens update of the least squares
+//
+// One solve = one thread-block cluster.  The cluster keeps w on chip (registers, vlen / (CS * 512) complex numbers
+// per thread) for the whole step.  Each v_i is streamed through shared memory exactly once: a 1-D bulk TMA copy
+// (cp.async.bulk + mbarrier) brings CTA r's contiguous slice of v_i into one of two buffers while the previous
+// slice is being used, the slice is dotted with w, the partial sums are exchanged through distributed shared memory
+// and one cluster barrier, and the same slice - still in shared memory - updates w.  HBM traffic per step is
+// (j + 3) V: read w, read v_0..v_j, write v_{j+1}; the paper's one-CUBLAS-call-per-dot/axpy schedule (made for a
+// GTX Titan) moves 5 V per basis vector, the two-sweep fallback in krylov.cu 2 V.
+//
+// Reductions are deterministic: fixed-shape warp trees, then fixed-order sums over warps and over cluster ranks.
+#include <cooperative_groups.h>
+#include <cstdint>
+
+#include "gsm_internal.cuh"
+#include "krylov_device.cuh"
+
+namespace cg = cooperative_groups;
+
+namespace gsm {
+
+#define MGS_T 512        // threads per CTA
+#define MGS_E 11         // complex elements of w per thread (registers)
+#define MGS_MAXCS 16     // largest cluster (non-portable size, opt-in)
+#define MGS_NW (MGS_T / 32)
+
+static __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+static __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+static __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+static __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+// 1-D bulk copy global -> this CTA's shared memory, completion signalled on the mbarrier (bytes % 16 == 0)
+static __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+static __device__ __forceinline__ double warp_sum_x(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+struct MgsSmem {
+    uint64_t mbar[2];
+    cplx red[2][MGS_MAXCS];   // red[parity][rank]: per-CTA partial sums, written by every rank through DSMEM
+    cplx wpart[MGS_NW];       // per-warp partial sums of this CTA
+};
+
+// Sum over the cluster of one complex number per thread.  `step` alternates the exchange buffer: a rank can be at
+// most one cluster barrier ahead of the slowest rank, so two buffers never collide.  Returns the same bits on every
+// thread of every CTA of the cluster.
+static __device__ __forceinline__ cplx cluster_sum(cg::cluster_group& cluster, MgsSmem* sm, cplx v, int step) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v.x = warp_sum_x(v.x);
+    v.y = warp_sum_x(v.y);
+    if (lane == 0) sm->wpart[warp] = v;
+    __syncthreads();
+    const unsigned cs = cluster.num_blocks(), rank = cluster.block_rank();
+    if (warp == 0) {
+        cplx t = make_double2(0.0, 0.0);
+        if (lane < MGS_NW) t = sm->wpart[lane];
+        t.x = warp_sum_x(t.x);
+        t.y = warp_sum_x(t.y);
+        if (lane < (int)cs) {
+            cplx* remote = cluster.map_shared_rank(&sm->red[step & 1][rank], lane);
+            *remote = t;
+        }
+    }
+    cluster.sync();
+    cplx tot = make_double2(0.0, 0.0);
+    for (unsigned c = 0; c < cs; ++c) {
+        const cplx q = sm->red[step & 1][c];
+        tot.x += q.x;
+        tot.y += q.y;
+    }
+    return tot;
+}
+
+// grid = batch * CS CTAs, cluster = CS CTAs along x; chunk = elements per CTA (<= MGS_T * MGS_E).
+__global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, KrylovState s, int batch, int j, int chunk) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const unsigned cs = cluster.num_blocks(), rank = cluster.block_rank();
+    const int b = blockIdx.x / cs;
+    if (!s.active[b]) return;   // uniform over the cluster: the flag only changes at the very end of this kernel
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    cplx* vbuf0 = reinterpret_cast<cplx*>(smem_raw);
+    cplx* vbuf1 = vbuf0 + chunk;
+    cplx* hsm = vbuf1 + chunk;                                   // [ld]   h_0..h_j of this step
+    cplx* snsm = hsm + d.ld;                                     // [mmax] previous rotations (rank 0 only)
+    double* cssm = reinterpret_cast<double*>(snsm + d.mmax);     // [mmax]
+    MgsSmem* sm = reinterpret_cast<MgsSmem*>(cssm + d.mmax + (d.mmax & 1));
+
+    const int t = threadIdx.x;
+    const long lo = (long)rank * chunk;
+    const int len = (int)max(0L, min((long)chunk, d.vlen - lo));
+    const uint32_t bytes = (uint32_t)len * (uint32_t)sizeof(cplx);
+    const long vs = (long)batch * d.vlen;
+    const cplx* vb = s.basis + (long)b * d.vlen + lo;            // slice of v_0; v_i at + i * vs
+    cplx* wg = s.basis + (long)b * d.vlen + (long)(j + 1) * vs + lo;
+
+    if (t == 0) {
+        mbar_init(&sm->mbar[0], 1);
+        mbar_init(&sm->mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (t == 0 && len > 0) {
+        mbar_expect_tx(&sm->mbar[0], bytes);
+        bulk_g2s(vbuf0, vb, bytes, &sm->mbar[0]);
+        if (j >= 1) {
+            mbar_expect_tx(&sm->mbar[1], bytes);
+            bulk_g2s(vbuf1, vb + vs, bytes, &sm->mbar[1]);
+        }
+    }
+    if (rank == 0)
+        for (int i = t; i < j; i += MGS_T) {
+            cssm[i] = s.cs[(long)b * d.mmax + i];
+            snsm[i] = s.sn[(long)b * d.mmax + i];
+        }
+    cplx w[MGS_E];
+#pragma unroll
+    for (int k = 0; k < MGS_E; ++k) {
+        const int e = k * MGS_T + t;
+        w[k] = (e < len) ? wg[e] : make_double2(0.0, 0.0);
+    }
+    // every CTA of the cluster must have started before any remote shared-memory write reaches it
+    cluster.sync();
+
+    uint32_t phase0 = 0, phase1 = 0;
+    for (int i = 0; i <= j; ++i) {
+        cplx* vbuf = (i & 1) ? vbuf1 : vbuf0;
+        if (len > 0) {
+            if (i & 1) { mbar_wait(&sm->mbar[1], phase1); phase1 ^= 1; }
+            else       { mbar_wait(&sm->mbar[0], phase0); phase0 ^= 1; }
+        }
+        cplx acc = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < MGS_E; ++k) {   // conj(v) * w
+            const int e = k * MGS_T + t;
+            if (e < len) {
+                const cplx v = vbuf[e];
+                acc.x = fma(v.x, w[k].x, fma(v.y, w[k].y, acc.x));
+                acc.y = fma(v.x, w[k].y, fma(-v.y, w[k].x, acc.y));
+            }
+        }
+        const cplx h = cluster_sum(cluster, sm, acc, i);
+#pragma unroll
+        for (int k = 0; k < MGS_E; ++k) {   // w -= h v
+            const int e = k * MGS_T + t;
+            if (e < len) {
+                const cplx v = vbuf[e];
+                w[k].x = fma(-h.x, v.x, fma(h.y, v.y, w[k].x));
+                w[k].y = fma(-h.x, v.y, fma(-h.y, v.x, w[k].y));
+            }
+        }
+        if (t == 0) hsm[i] = h;
+        __syncthreads();   // every thread is done with vbuf: it may be refilled
+        if (t == 0 && len > 0 && i + 2 <= j) {
+            uint64_t* bar = &sm->mbar[i & 1];
+            mbar_expect_tx(bar, bytes);
+            bulk_g2s(vbuf, vb + (long)(i + 2) * vs, bytes, bar);
+        }
+    }
+    cplx nn = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < MGS_E; ++k) nn.x = fma(w[k].x, w[k].x, fma(w[k].y, w[k].y, nn.x));
+    nn = cluster_sum(cluster, sm, nn, j + 1);
+    const double hn = sqrt(nn.x);
+    const double sc = hn > 0.0 ? 1.0 / hn : 0.0;
+#pragma unroll
+    for (int k = 0; k < MGS_E; ++k) {
+        const int e = k * MGS_T + t;
+        if (e < len) wg[e] = make_double2(w[k].x * sc, w[k].y * sc);
+    }
+    if (rank == 0 && t == 0) givens_step(d, s, b, j, hsm, hn, cssm, snsm);
+}
+
+size_t arnoldi_cluster_smem(const KrylovDims& d, int chunk) {
+    return sizeof(cplx) * (2 * (size_t)chunk + d.ld + d.mmax) + sizeof(double) * (d.mmax + (d.mmax & 1)) +
+           sizeof(MgsSmem) + 128;
+}
+
+// Smallest power-of-two cluster whose CTAs can each keep their slice of w in registers; 0 if the vector is too long
+// or the device cannot co-schedule such a cluster (then krylov.cu's two-sweep path is used).
+cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out) {
+    *cs_out = 0;
+    *chunk_out = 0;
+    const long cap = (long)MGS_T * MGS_E;
+    int cs = 1;
+    while (cs <= MGS_MAXCS && (d.vlen + cs - 1) / cs > cap) cs *= 2;
+    if (cs > MGS_MAXCS) return cudaSuccess;
+    const int chunk = (int)((d.vlen + cs - 1) / cs);
+    const size_t smem = arnoldi_cluster_smem(d, chunk);
+    if (smem > 227 * 1024) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (cs > 8) {
+        e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) { cudaGetLastError(); return cudaSuccess; }
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cs);
+    cfg.blockDim = dim3(MGS_T);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cs;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    int nclusters = 0;
+    e = cudaOccupancyMaxActiveClusters(&nclusters, arnoldi_mgs_kernel, &cfg);
+    if (e != cudaSuccess || nclusters < 1) { cudaGetLastError(); return cudaSuccess; }
+    *cs_out = cs;
+    *chunk_out = chunk;
+    return cudaSuccess;
+}
+
+cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
+                                   cudaStream_t st, Profiler* prof, int nact) {
+    ProfScope ps_(prof, KC_ARNOLDI_MGS, st, 16.0 * d.vlen * (j + 3.0) * nact);   // reads w, v_0..v_j; writes v_{j+1}
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)batch * cs);
+    cfg.blockDim = dim3(MGS_T);
+    cfg.dynamicSmemBytes = arnoldi_cluster_smem(d, chunk);
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cs;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, arnoldi_mgs_kernel, d, s, batch, j, chunk);
+}
+
+}  // namespace gsm

@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -19,6 +20,7 @@ struct gsm_plan {
     cudaStream_t stream = nullptr;
     int max_batch = 1, max_iters = 64;
     long i0 = 0;                  // flat index of m = 0 inside one component
+    int mgs_cs = 0, mgs_chunk = 0; // cluster MGS Arnoldi step (0 = two-sweep fallback)
     std::vector<void*> allocs;    // every device allocation, freed in destroy
     long long device_bytes = 0;
     Profiler prof;
@@ -267,6 +269,8 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         kd.mmax = m;
         kd.ld = m + 1;
         KrylovState& ks = plan->ks;
+        CK(arnoldi_cluster_plan(kd, &plan->mgs_cs, &plan->mgs_chunk));
+        if (getenv("GSM_FORCE_TWO_SWEEP")) plan->mgs_cs = 0;
         CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
         CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &plan->ybuf, (size_t)B * kd.vlen));
@@ -404,11 +408,15 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     for (; j < kd.mmax; ++j) {
         CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
                         plan->W, ks.active, st, prof, nact));
-        CK(launch_sweep_dots(kd, ks, nb, j, st, prof, nact));
-        CK(launch_hsolve(kd, ks, nb, j, st, prof));
-        CK(launch_sweep_update(kd, ks, nb, j, st, prof, nact));
-        CK(launch_givens(kd, ks, nb, j, st, prof));
-        CK(launch_normalize(kd, ks, nb, j, st, prof, nact));
+        if (plan->mgs_cs > 0) {
+            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, st, prof, nact));
+        } else {
+            CK(launch_sweep_dots(kd, ks, nb, j, st, prof, nact));
+            CK(launch_hsolve(kd, ks, nb, j, st, prof));
+            CK(launch_sweep_update(kd, ks, nb, j, st, prof, nact));
+            CK(launch_givens(kd, ks, nb, j, st, prof));
+            CK(launch_normalize(kd, ks, nb, j, st, prof, nact));
+        }
         CK(cudaMemcpyAsync(pin_i, ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         nact = pin_i[0];
@@ -479,7 +487,7 @@ extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, 
 namespace gsm {
 static const char* const kKernelClassNames[KC_COUNT] = {
     "z_forward", "xy_conv", "z_inverse_green", "sweep_dots", "hsolve", "sweep_update", "givens", "normalize",
-    "combine", "residual", "small", "plan"};
+    "arnoldi_mgs", "combine", "residual", "small", "plan"};
 const char* kernel_class_name(int cls) { return cls >= 0 && cls < KC_COUNT ? kKernelClassNames[cls] : ""; }
 
 void Profiler::begin(int c, cudaStream_t st, double nbytes) {

@@ -12,7 +12,7 @@ namespace gsm {
 // Kernel classes for launch counting and (optional) per-class CUDA-event timing (gsm_plan_profile).
 enum KernelClass {
     KC_Z_FORWARD = 0, KC_XY_CONV, KC_Z_INVERSE_GREEN, KC_SWEEP_DOTS, KC_HSOLVE, KC_SWEEP_UPDATE, KC_GIVENS,
-    KC_NORMALIZE, KC_COMBINE, KC_RESIDUAL, KC_SMALL, KC_PLAN, KC_COUNT
+    KC_NORMALIZE, KC_ARNOLDI_MGS, KC_COMBINE, KC_RESIDUAL, KC_SMALL, KC_PLAN, KC_COUNT
 };
 const char* kernel_class_name(int cls);
 
@@ -122,5 +122,12 @@ cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch,
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
                                  double* d_resid, cudaStream_t st, Profiler* prof);
 cudaError_t krylov_init_attributes();
+
+// ---- launches implemented in arnoldi_cluster.cu ------------------------------------------------------------------
+// One Arnoldi step (MGS + norm + normalise + Givens) per solve in one thread-block cluster, basis read once.
+// arnoldi_cluster_plan: cluster size (0 = not usable: fall back to the two-sweep kernels) and elements per CTA.
+cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out);
+cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
+                                   cudaStream_t st, Profiler* prof, int nact);
 
 }  // namespace gsm

@@ -12,6 +12,7 @@
 //
 // <u, v> = sum conj(u) v.  Reductions are two-stage and deterministic (per-CTA partials, then a fixed-order sum).
 #include "gsm_internal.cuh"
+#include "krylov_device.cuh"
 
 namespace gsm {
 
@@ -178,51 +179,13 @@ __global__ void __launch_bounds__(KT) sweep_update_kernel(KrylovDims d, KrylovSt
     }
 }
 
-// per solve: h_{j+1,j} = ||w||, Givens least squares (Saad Alg. 6.9 / 6.5.3), residual estimate, stop test
+// two-sweep path: h_{j+1,j} = ||w|| from the partial norms of sweep 2, then the Givens step
 __global__ void givens_kernel(KrylovDims d, KrylovState s, int batch, int j) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch || !s.active[b]) return;
     double nn = 0.0;
     for (int c = 0; c < d.nchunk; ++c) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
-    const double hn = sqrt(nn);
-    cplx* Rc = s.R + (long)b * d.ld * d.mmax;     // Rc[i * mmax + j]
-    const cplx* h = s.hcol + (long)b * d.ld;
-    double* cs = s.cs + (long)b * d.mmax;
-    cplx* sn = s.sn + (long)b * d.mmax;
-    cplx* g = s.g + (long)b * d.ld;
-    cplx hi = h[0];
-    for (int i = 0; i < j; ++i) {   // previous rotations on the new column
-        const cplx hn1 = h[i + 1];
-        const cplx t = cadd(make_double2(cs[i] * hi.x, cs[i] * hi.y), cmul(sn[i], hn1));
-        const cplx u = csub(make_double2(cs[i] * hn1.x, cs[i] * hn1.y), cmulc(hi, sn[i]));   // -conj(sn) hi + cs hn1
-        Rc[(long)i * d.mmax + j] = t;
-        hi = u;
-    }
-    const cplx a = hi;
-    const double aa = hypot(a.x, a.y);
-    const double r = hypot(aa, hn);
-    double c;
-    cplx sv;
-    if (r == 0.0) { c = 1.0; sv = make_double2(0.0, 0.0); }
-    else if (aa == 0.0) { c = 0.0; sv = make_double2(1.0, 0.0); }
-    else { c = aa / r; sv = make_double2(a.x / aa * hn / r, a.y / aa * hn / r); }   // (a/|a|) conj(hn)/r, hn real
-    cs[j] = c;
-    sn[j] = sv;
-    Rc[(long)j * d.mmax + j] = cadd(make_double2(c * a.x, c * a.y), make_double2(sv.x * hn, sv.y * hn));
-    const cplx gj = g[j];
-    g[j + 1] = make_double2(-(sv.x * gj.x + sv.y * gj.y), -(sv.x * gj.y - sv.y * gj.x));   // -conj(sn) g_j
-    g[j] = make_double2(c * gj.x, c * gj.y);
-    const double beta = s.beta[b];
-    const double res = hypot(g[j + 1].x, g[j + 1].y) / beta;
-    s.hist[(long)b * d.mmax + j] = res;
-    s.iters[b] = j + 1;
-    const bool lucky = hn <= 2.220446049250313e-16 * beta;
-    if (res <= s.tol[0] || lucky) {
-        s.active[b] = 0;
-        atomicSub(s.nactive, 1);
-    } else {
-        s.scale[b] = 1.0 / hn;
-    }
+    givens_step(d, s, b, j, s.hcol + (long)b * d.ld, sqrt(nn), s.cs + (long)b * d.mmax, s.sn + (long)b * d.mmax);
 }
 
 // v_{j+1} = w / h_{j+1,j}
