@@ -8,7 +8,7 @@
 // per thread) for the whole step.  Each v_i is streamed through shared memory exactly once: a 1-D bulk TMA copy
 // (cp.async.bulk + mbarrier) brings CTA r's contiguous slice of v_i into one of two buffers while the previous
 // slice is being used, the slice is dotted with w, the partial sums are exchanged through distributed shared memory
-// and one cluster barrier, and the same slice - still in shared memory - updates w.  HBM traffic per step is
+// (st.async + mbarrier, no cluster-wide barrier), and the same slice - still in shared memory - updates w.  HBM traffic per step is
 // (j + 3) V: read w, read v_0..v_j, write v_{j+1}; the paper's one-CUBLAS-call-per-dot/axpy schedule (made for a
 // GTX Titan) moves 5 V per basis vector, the two-sweep fallback in krylov.cu 2 V.
 //
@@ -55,40 +55,56 @@ static __device__ __forceinline__ double warp_sum_x(double v) {
     return v;
 }
 
+// address of the same shared-memory variable in CTA `rank` of the cluster (shared::cluster window)
+static __device__ __forceinline__ uint32_t map_rank(uint32_t cta_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
+    return r;
+}
+// 16-byte asynchronous store into a peer CTA's shared memory that also completes 16 bytes on the peer's mbarrier:
+// the data is visible to whoever observes the mbarrier phase flip, with no cluster-wide barrier or fence.
+static __device__ __forceinline__ void st_async_cplx(uint32_t remote_addr, cplx v, uint32_t remote_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(remote_addr), "d"(v.x), "d"(v.y), "r"(remote_bar) : "memory");
+}
+
 struct MgsSmem {
-    uint64_t mbar[2];
+    uint64_t mbar[2];         // TMA completion of the two basis-slice buffers
+    uint64_t rbar[2];         // arrival of the CS partial sums of an exchange (even / odd exchange number)
     cplx red[2][MGS_MAXCS];   // red[parity][rank]: per-CTA partial sums, written by every rank through DSMEM
     cplx wpart[MGS_NW];       // per-warp partial sums of this CTA
 };
 
-// Sum over the cluster of one complex number per thread.  `step` alternates the exchange buffer: a rank can be at
-// most one cluster barrier ahead of the slowest rank, so two buffers never collide.  Returns the same bits on every
-// thread of every CTA of the cluster.
-static __device__ __forceinline__ cplx cluster_sum(cg::cluster_group& cluster, MgsSmem* sm, cplx v, int step) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+// Sum over the cluster of one complex number per thread; exchange number `step` (0, 1, 2, ... in program order).
+// Every rank sends its CTA-level partial to all ranks with st.async, which completes bytes on the receiver's
+// mbarrier; the receiver waits for CS * 16 bytes.  Exchanges alternate between two (mbarrier, buffer) pairs: rank X
+// can only send exchange s+2 after it has received every rank's exchange s+1, which rank Y sends after all of its
+// threads have consumed exchange s - so two pairs never collide.  All ranks sum the same values in the same fixed
+// tree order: identical bits everywhere, deterministic.
+static __device__ __forceinline__ cplx cluster_sum(MgsSmem* sm, cplx v, int step, unsigned cs, unsigned rank) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, par = step & 1;
     v.x = warp_sum_x(v.x);
     v.y = warp_sum_x(v.y);
     if (lane == 0) sm->wpart[warp] = v;
     __syncthreads();
-    const unsigned cs = cluster.num_blocks(), rank = cluster.block_rank();
     if (warp == 0) {
+        if (lane == 0) mbar_expect_tx(&sm->rbar[par], cs * (uint32_t)sizeof(cplx));
         cplx t = make_double2(0.0, 0.0);
         if (lane < MGS_NW) t = sm->wpart[lane];
         t.x = warp_sum_x(t.x);
         t.y = warp_sum_x(t.y);
-        if (lane < (int)cs) {
-            cplx* remote = cluster.map_shared_rank(&sm->red[step & 1][rank], lane);
-            *remote = t;
-        }
+        if (lane < (int)cs)
+            st_async_cplx(map_rank(smem_u32(&sm->red[par][rank]), lane), t, map_rank(smem_u32(&sm->rbar[par]), lane));
     }
-    cluster.sync();
-    cplx tot = make_double2(0.0, 0.0);
-    for (unsigned c = 0; c < cs; ++c) {
-        const cplx q = sm->red[step & 1][c];
-        tot.x += q.x;
-        tot.y += q.y;
-    }
-    return tot;
+    mbar_wait(&sm->rbar[par], (step >> 1) & 1);
+    cplx q[MGS_MAXCS];
+#pragma unroll
+    for (int c = 0; c < MGS_MAXCS; ++c) q[c] = (c < (int)cs) ? sm->red[par][c] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int w = 1; w < MGS_MAXCS; w *= 2)
+#pragma unroll
+        for (int c = 0; c + w < MGS_MAXCS; c += 2 * w) { q[c].x += q[c + w].x; q[c].y += q[c + w].y; }
+    return q[0];
 }
 
 // grid = batch * CS CTAs, cluster = CS CTAs along x; chunk = elements per CTA (<= MGS_T * MGS_E).
@@ -117,6 +133,8 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     if (t == 0) {
         mbar_init(&sm->mbar[0], 1);
         mbar_init(&sm->mbar[1], 1);
+        mbar_init(&sm->rbar[0], 1);
+        mbar_init(&sm->rbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -139,7 +157,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
         const int e = k * MGS_T + t;
         w[k] = (e < len) ? wg[e] : make_double2(0.0, 0.0);
     }
-    // every CTA of the cluster must have started before any remote shared-memory write reaches it
+    // every CTA of the cluster must have started (mbarriers initialised) before any remote write reaches it
     cluster.sync();
 
     uint32_t phase0 = 0, phase1 = 0;
@@ -159,7 +177,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
                 acc.y = fma(v.x, w[k].y, fma(-v.y, w[k].x, acc.y));
             }
         }
-        const cplx h = cluster_sum(cluster, sm, acc, i);
+        const cplx h = cluster_sum(sm, acc, i, cs, rank);
 #pragma unroll
         for (int k = 0; k < MGS_E; ++k) {   // w -= h v
             const int e = k * MGS_T + t;
@@ -180,7 +198,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     cplx nn = make_double2(0.0, 0.0);
 #pragma unroll
     for (int k = 0; k < MGS_E; ++k) nn.x = fma(w[k].x, w[k].x, fma(w[k].y, w[k].y, nn.x));
-    nn = cluster_sum(cluster, sm, nn, j + 1);
+    nn = cluster_sum(sm, nn, j + 1, cs, rank);
     const double hn = sqrt(nn.x);
     const double sc = hn > 0.0 ? 1.0 / hn : 0.0;
 #pragma unroll
@@ -189,6 +207,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
         if (e < len) wg[e] = make_double2(w[k].x * sc, w[k].y * sc);
     }
     if (rank == 0 && t == 0) givens_step(d, s, b, j, hsm, hn, cssm, snsm);
+    cluster.sync();   // no CTA leaves while a peer's asynchronous store to it could still be in flight
 }
 
 size_t arnoldi_cluster_smem(const KrylovDims& d, int chunk) {
