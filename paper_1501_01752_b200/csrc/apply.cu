@@ -178,7 +178,8 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
     { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
       z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active); }
     { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
-      xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); }
+      if (g.chat64) launch_xy_conv64(g, batch, d_W, g.chat64, d_active, st);
+      else xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); }
     { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
       z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); }
     return cudaGetLastError();
@@ -191,6 +192,7 @@ cudaError_t apply_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(z_forward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(xy_conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = apply64_init_attributes();
     return e;
 }
 }  // namespace gsm

@@ -1,0 +1,187 @@
+// apply64.cu - operator-apply passes specialised for a 64-point axis (17..32 harmonics kept, e.g. the 31^3 configs of
+// BASELINE.json), same data layouts and the same radix-8 x radix-8 network as the generic kernels of apply.cu
+// (Toeplitz product by FFT).
+//
+// Eight lanes share one line: lane u of the group runs butterfly u of both stages with its 8 points in registers.
+//   forward  stage 1: inputs e = u + 8p (only p < 4 can be non-zero: the padding half is never loaded or added),
+//                     outputs y_q w64^(u q) for e = u + 8q; the 7 twiddles depend on (u, q) only and live in
+//                     registers for the whole kernel;
+//            exchange: an 8 x 8 transpose inside the group through a warp-private scratch line (padded index
+//                     e + e/8, conflict-free both ways) fenced by __syncwarp only;
+//            stage 2: inputs e = 8u + p, no twiddles, outputs at positions 8u + q.
+//   inverse = mirror image; its last stage forms only the 4 outputs that are kept.
+// A 64 x 64 plane therefore needs two block-wide barriers (y <-> x hand-over), not one per stage, no index
+// division, and no twiddle traffic.
+#include "gsm_internal.cuh"
+
+namespace gsm {
+
+// forward radix-8 with a[4..7] == 0 on entry (zero padding): the first layer of adds disappears
+static __device__ __forceinline__ void bfly8_fwd_half_in(cplx* a) {
+    // even part from {a0, a2, 0, 0}, odd part from {a1, a3, 0, 0}
+    const cplx e0 = cadd(a[0], a[2]), e2 = csub(a[0], a[2]);
+    const cplx m2 = mul_mi<false>(a[2]);
+    const cplx e1 = cadd(a[0], m2), e3 = csub(a[0], m2);
+    const cplx o0 = cadd(a[1], a[3]), o2r = csub(a[1], a[3]);
+    const cplx m3 = mul_mi<false>(a[3]);
+    const cplx o1r = cadd(a[1], m3), o3r = csub(a[1], m3);
+    // o[k] *= w8^k, w8 = exp(-i pi/4)
+    const cplx o1 = make_double2((o1r.x + o1r.y) * GSM_SQRT1_2, (o1r.y - o1r.x) * GSM_SQRT1_2);
+    const cplx o2 = mul_mi<false>(o2r);
+    const cplx o3 = make_double2((o3r.y - o3r.x) * GSM_SQRT1_2, (-o3r.x - o3r.y) * GSM_SQRT1_2);
+    a[0] = cadd(e0, o0);  a[4] = csub(e0, o0);
+    a[1] = cadd(e1, o1);  a[5] = csub(e1, o1);
+    a[2] = cadd(e2, o2);  a[6] = csub(e2, o2);
+    a[3] = cadd(e3, o3);  a[7] = csub(e3, o3);
+}
+
+// inverse radix-8 producing only outputs 0..3 (the kept half)
+static __device__ __forceinline__ void bfly8_inv_half_out(cplx* a) {
+    cplx e[4] = {a[0], a[2], a[4], a[6]};
+    cplx o[4] = {a[1], a[3], a[5], a[7]};
+    Bfly<4, true>::run(e);
+    Bfly<4, true>::run(o);
+    const cplx o1 = make_double2((o[1].x - o[1].y) * GSM_SQRT1_2, (o[1].y + o[1].x) * GSM_SQRT1_2);
+    const cplx o2 = mul_mi<true>(o[2]);
+    const cplx o3 = make_double2((-o[3].x - o[3].y) * GSM_SQRT1_2, (o[3].x - o[3].y) * GSM_SQRT1_2);
+    a[0] = cadd(e[0], o[0]);
+    a[1] = cadd(e[1], o1);
+    a[2] = cadd(e[2], o2);
+    a[3] = cadd(e[3], o3);
+}
+
+#define SC_LINE 72   // padded scratch line: element e lives at e + e/8
+
+// forward 64-point transform of one line held by an 8-lane group.  In: a[0..3] = x[u + 8p] (a[4..7] ignored).
+// Out: a[q] = value at position 8u + q.  sc = this line's scratch (SC_LINE complex numbers, warp-private).
+static __device__ __forceinline__ void fwd64_group(cplx* a, const cplx* tw, cplx* sc, int u) {
+    bfly8_fwd_half_in(a);
+    sc[u] = a[0];
+#pragma unroll
+    for (int q = 1; q < 8; ++q) sc[u + 9 * q] = cmul(a[q], tw[q - 1]);
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 8; ++p) a[p] = sc[9 * u + p];
+    Bfly<8, false>::run(a);
+}
+
+// inverse 64-point transform.  In: a[q] = value at position 8u + q.  Out: a[0..3] = y[u + 8p], p < 4.
+static __device__ __forceinline__ void inv64_group(cplx* a, const cplx* tw, cplx* sc, int u) {
+    Bfly<8, true>::run(a);
+#pragma unroll
+    for (int p = 0; p < 8; ++p) sc[9 * u + p] = a[p];
+    __syncwarp();
+    a[0] = sc[u];
+#pragma unroll
+    for (int q = 1; q < 8; ++q) a[q] = cmulc(sc[u + 9 * q], tw[q - 1]);
+    bfly8_inv_half_out(a);
+    __syncwarp();   // the scratch line is free for the next transform
+}
+
+static __device__ __forceinline__ void load_group_twiddles(cplx* tw, const cplx* __restrict__ table, int u) {
+#pragma unroll
+    for (int q = 1; q < 8; ++q) tw[q - 1] = __ldg(table + ((u * q) & 63));
+}
+
+// ------------------------------------------------------------------------------------------- pass 2, P1 = P2 = 64
+// One CTA per (solve b, component c, z-position pos3) plane, 8 warps.  A[r][col]: row r = y-position (64), 32 columns
+// = x-index i1 rotated by r/8, so that both the y-phase (lanes differ in u = r/8) and the x-phase (lanes differ in
+// i1) touch 8 distinct 16-byte bank groups per quarter-warp.
+//   y forward : group (i1 = 4 warp + ln) reads its 4 x 8 inputs straight from W (contiguous in i2), writes rows of A
+//   x         : group (row r) reads <= 32 inputs from A, forward, * Chat, inverse, writes the kept 32 back in place
+//   y inverse : mirror of y forward, stores straight to W
+// chat64 is Chat permuted so that the 8 lanes of a group read 8 consecutive coefficients:
+//   chat64[((pos3 * 64 + r) * 8 + q) * 8 + u] = Chat[pos3][pos1 = 8u + q][pos2 = r].
+__global__ void __launch_bounds__(256, 3) xy_conv64_kernel(ApplyGeom g, cplx* __restrict__ W,
+                                                           const cplx* __restrict__ chat64,
+                                                           const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y, pos3 = blockIdx.x;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* A = reinterpret_cast<cplx*>(smem_raw);   // [64][32]
+    cplx* scratch = A + 64 * 32;                   // [32 lines][SC_LINE]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, u = lane & 7, ln = lane >> 3;
+    const int N1 = g.N1, N2 = g.N2;
+    cplx tw[7];
+    load_group_twiddles(tw, g.tw[0], u);
+    cplx* sc = scratch + (warp * 4 + ln) * SC_LINE;
+    cplx* Wp = W + (((long)b * 3 + c) * 64 + pos3) * g.NL;
+    cplx a[8];
+
+    {   // ---- y forward
+        const int i1 = warp * 4 + ln;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int i2 = u + 8 * p;
+            a[p] = (i1 < N1 && i2 < N2) ? Wp[i1 * N2 + i2] : make_double2(0.0, 0.0);
+        }
+        fwd64_group(a, tw, sc, u);
+        const int col = (i1 + u) & 31;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) A[(8 * u + q) * 32 + col] = a[q];
+    }
+    __syncthreads();
+    // ---- x: forward, multiply by the coefficient spectrum, inverse
+#pragma unroll 1
+    for (int round = 0; round < 2; ++round) {
+        const int r = (round * 8 + warp) * 4 + ln;
+        cplx* Ar = A + r * 32;
+        const int rot = r >> 3;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int i1 = u + 8 * p;
+            a[p] = (i1 < N1) ? Ar[(i1 + rot) & 31] : make_double2(0.0, 0.0);
+        }
+        fwd64_group(a, tw, sc, u);
+        const cplx* cp = chat64 + ((long)(pos3 * 64 + r) * 64) + u;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], __ldg(cp + 8 * q));
+        inv64_group(a, tw, sc, u);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int i1 = u + 8 * p;
+            if (i1 < N1) Ar[(i1 + rot) & 31] = a[p];
+        }
+    }
+    __syncthreads();
+    {   // ---- y inverse
+        const int i1 = warp * 4 + ln;
+        const int col = (i1 + u) & 31;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) a[q] = A[(8 * u + q) * 32 + col];
+        inv64_group(a, tw, sc, u);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int i2 = u + 8 * p;
+            if (i1 < N1 && i2 < N2) Wp[i1 * N2 + i2] = a[p];
+        }
+    }
+}
+
+__global__ void chat64_layout_kernel(const cplx* __restrict__ chat, cplx* __restrict__ chat64) {
+    const long total = 64L * 64 * 64;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const int u = (int)(i & 7), q = (int)((i >> 3) & 7), r = (int)((i >> 6) & 63), p3 = (int)(i >> 12);
+        chat64[i] = chat[((long)p3 * 64 + (8 * u + q)) * 64 + r];
+    }
+}
+
+static const size_t XY64_SMEM = sizeof(cplx) * (64 * 32 + 32 * SC_LINE);
+
+bool apply64_usable(const ApplyGeom& g) {
+    return g.ax[0].P == 64 && g.ax[1].P == 64 && g.ax[2].P == 64 && g.N1 <= 32 && g.N2 <= 32 && g.N3 <= 32;
+}
+cudaError_t launch_chat64_layout(const cplx* d_chat, cplx* d_chat64, cudaStream_t st) {
+    chat64_layout_kernel<<<1024, 256, 0, st>>>(d_chat, d_chat64);
+    return cudaGetLastError();
+}
+cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat64, const int* d_active,
+                             cudaStream_t st) {
+    xy_conv64_kernel<<<dim3(64, 3, batch), 256, XY64_SMEM, st>>>(g, d_W, d_chat64, d_active);
+    return cudaGetLastError();
+}
+cudaError_t apply64_init_attributes() {
+    return cudaFuncSetAttribute(xy_conv64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
+}
+
+}  // namespace gsm

@@ -24,6 +24,7 @@ struct gsm_plan {
     std::vector<void*> allocs;    // every device allocation, freed in destroy
     long long device_bytes = 0;
     Profiler prof;
+    cplx* chat64 = nullptr;
     cplx *coef = nullptr, *chat = nullptr, *pad = nullptr, *W = nullptr, *xbuf = nullptr, *ybuf = nullptr;
     size_t vgrid_count = 0;
     cplx* vgrid = nullptr;        // voxel path: device copy of the grid, transformed in place
@@ -209,6 +210,11 @@ static gsm_status build_spectrum(gsm_plan* plan) {
     if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0], full[1], P[2], g.tw[1], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(pad, 1, full[0], (long)P[1] * P[2], g.tw[0], plan->stream);
     if (e == cudaSuccess) e = launch_chat_layout(pad, P, plan->chat, plan->stream);
+    if (e == cudaSuccess && apply64_usable(g) && !getenv("GSM_GENERIC_APPLY")) {
+        if (!plan->chat64) CK(dalloc(plan, &plan->chat64, np));
+        e = launch_chat64_layout(plan->chat, plan->chat64, plan->stream);
+        g.chat64 = plan->chat64;
+    }
     CK(e);
     g.chat = plan->chat;
     return GSM_OK;

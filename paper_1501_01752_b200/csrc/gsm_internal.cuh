@@ -51,6 +51,7 @@ struct ApplyGeom {
     int CB, CBs;         // columns per x-batch in pass 2 and the odd row stride (>= CB) of its scratch
     const cplx* tw[3];   // device twiddle tables exp(-2 pi i k / P_a)
     const cplx* chat;    // coefficient spectrum, position order, [P3][P1][P2], scaled by 1/(P1 P2 P3)
+    const cplx* chat64;  // same, permuted for apply64.cu (null unless apply64_usable)
     double K[3];         // 2 pi / Lambda_a
     int mmin[3];         // lowest order per axis
     double epsb_re, epsb_im;
@@ -71,6 +72,12 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
                          cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact);
 size_t apply_smem_max(const ApplyGeom& g);
 cudaError_t apply_init_attributes();
+// apply64.cu: passes specialised for 64-point axes (chat64 = Chat permuted for 8-lane groups)
+bool apply64_usable(const ApplyGeom& g);
+cudaError_t apply64_init_attributes();
+cudaError_t launch_chat64_layout(const cplx* d_chat, cplx* d_chat64, cudaStream_t st);
+cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat64, const int* d_active,
+                             cudaStream_t st);
 cudaError_t plan_init_attributes();
 
 // plan-time (a0): coefficients and their spectrum
