@@ -176,12 +176,14 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
     const double V = 16.0 * 3.0 * g.n * nact, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL * nact;
     const double Cb = 16.0 * g.ax[0].P * g.ax[1].P * g.ax[2].P;
     { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
-      z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active); }
+      if (g.chat64) launch_z_forward64(g, batch, d_x, d_W, d_active, st);
+      else z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active); }
     { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
       if (g.chat64) launch_xy_conv64(g, batch, d_W, g.chat64, d_active, st);
       else xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); }
     { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
-      z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); }
+      if (g.chat64) launch_z_inverse_green64(g, batch, d_W, d_x, d_y, d_kvec, d_k0, d_active, st);
+      else z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); }
     return cudaGetLastError();
 }
 

@@ -158,6 +158,135 @@ __global__ void __launch_bounds__(256, 3) xy_conv64_kernel(ApplyGeom g, cplx* __
     }
 }
 
+// ------------------------------------------------------------------------------------------- pass 1, P3 = 64
+// CTA = 32 consecutive z-lines of one (b, c).  Each group loads its line's <= 32 inputs straight from x (contiguous),
+// transforms, and drops the 64 outputs into a [pos3][32 lines] tile (columns rotated by pos3/8: conflict-free), which
+// is then written to W[b][c][pos3][l] as 512-byte rows.
+__global__ void __launch_bounds__(256, 3) z_forward64_kernel(ApplyGeom g, const cplx* __restrict__ x, cplx* __restrict__ W,
+                                                             const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* T = reinterpret_cast<cplx*>(smem_raw);   // [64][32]
+    cplx* scratch = T + 64 * 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, u = lane & 7, ln = lane >> 3;
+    const int N3 = g.N3, NL = g.NL;
+    cplx tw[7];
+    load_group_twiddles(tw, g.tw[2], u);
+    cplx* sc = scratch + (warp * 4 + ln) * SC_LINE;
+    const int l0 = blockIdx.x * 32, line = warp * 4 + ln, l = l0 + line;
+    const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l * N3;
+    cplx a[8];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const int i3 = u + 8 * p;
+        a[p] = (l < NL && i3 < N3) ? xs[i3] : make_double2(0.0, 0.0);
+    }
+    fwd64_group(a, tw, sc, u);
+    const int col = (line + u) & 31;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) T[(8 * u + q) * 32 + col] = a[q];
+    __syncthreads();
+    cplx* Wd = W + ((long)b * 3 + c) * 64 * NL + l0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int r = k * 8 + warp;                       // one 512-byte row per warp and step
+        const int ll = (lane - (r >> 3)) & 31;            // logical line stored in physical column `lane`
+        if (l0 + ll < NL) Wd[(long)r * NL + ll] = T[r * 32 + lane];
+    }
+}
+
+// ------------------------------------------------------------------------------------------- pass 3, P3 = 64
+// CTA = 32 consecutive z-lines, all three components.  The [pos3][32 lines] tiles of W arrive by cp.async (16 bytes
+// per request, columns rotated like pass 1), double-buffered over the components; each group inverse-transforms its
+// line, keeps the <= 4 x 3 kept outputs in registers and applies the Green dyadic of Eq. 4:
+//   y_c = x_c - (k_b^2 F_c - k_c (k.F)) / (k.k - k_b^2),  k = k_inc + m o K  (unconjugated k.k).
+static __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+static __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> static __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__global__ void __launch_bounds__(256, 2) z_inverse_green64_kernel(ApplyGeom g, const cplx* __restrict__ W,
+                                                                   const cplx* __restrict__ x, cplx* __restrict__ y,
+                                                                   const double* __restrict__ kvec,
+                                                                   const double* __restrict__ k0s,
+                                                                   const int* __restrict__ active) {
+    const int b = blockIdx.y;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* T0 = reinterpret_cast<cplx*>(smem_raw);   // two [64][32] tiles
+    cplx* T1 = T0 + 64 * 32;
+    cplx* scratch = T1 + 64 * 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, u = lane & 7, ln = lane >> 3;
+    const int N3 = g.N3, NL = g.NL;
+    const int l0 = blockIdx.x * 32, line = warp * 4 + ln, l = l0 + line;
+    auto load_tile = [&](cplx* T, int c) {
+        const cplx* Ws = W + ((long)b * 3 + c) * 64 * NL + l0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int r = k * 8 + warp;
+            const int ll = (lane - (r >> 3)) & 31;
+            if (l0 + ll < NL) cp_async16(&T[r * 32 + lane], Ws + (long)r * NL + ll);
+        }
+        cp_async_commit();
+    };
+    load_tile(T0, 0);
+    load_tile(T1, 1);
+    cplx tw[7];
+    load_group_twiddles(tw, g.tw[2], u);
+    cplx* sc = scratch + (warp * 4 + ln) * SC_LINE;
+    const int col = (line + u) & 31;
+    cplx F[3][4];
+    cplx a[8];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (c < 2) cp_async_wait<1>(); else cp_async_wait<0>();
+        __syncthreads();
+        const cplx* T = (c & 1) ? T1 : T0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) a[q] = T[(8 * u + q) * 32 + col];
+        if (c == 0) {           // tile 0 is consumed: refill it with component 2
+            __syncthreads();
+            load_tile(T0, 2);
+        }
+        inv64_group(a, tw, sc, u);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) F[c][p] = a[p];
+    }
+    if (l >= NL) return;
+    const double k0 = k0s[b];
+    const double kb2r = k0 * k0 * g.epsb_re, kb2i = k0 * k0 * g.epsb_im;
+    const int i1 = l / g.N2, i2 = l - i1 * g.N2;
+    const double k1 = kvec[3 * b + 0] + (i1 + g.mmin[0]) * g.K[0];
+    const double k2 = kvec[3 * b + 1] + (i2 + g.mmin[1]) * g.K[1];
+    const double k12 = k1 * k1 + k2 * k2;
+    const long base = (long)b * 3 * g.n + (long)l * N3;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const int i3 = u + 8 * p;
+        if (i3 >= N3) continue;
+        const double k3 = kvec[3 * b + 2] + (i3 + g.mmin[2]) * g.K[2];
+        const cplx F0 = F[0][p], F1 = F[1][p], F2 = F[2][p];
+        const cplx s = make_double2(k1 * F0.x + k2 * F1.x + k3 * F2.x, k1 * F0.y + k2 * F1.y + k3 * F2.y);
+        const double dr = k12 + k3 * k3 - kb2r, di = -kb2i;
+        const double inv = 1.0 / (dr * dr + di * di);
+        const cplx rden = make_double2(dr * inv, -di * inv);   // 1 / (k.k - k_b^2)
+        const cplx kb2 = make_double2(kb2r, kb2i);
+        const double kk[3] = {k1, k2, k3};
+        const cplx Fc[3] = {F0, F1, F2};
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            cplx num = cmul(kb2, Fc[c]);
+            num.x -= kk[c] * s.x;
+            num.y -= kk[c] * s.y;
+            const cplx q = cmul(num, rden);
+            const cplx xv = x[base + c * g.n + i3];
+            y[base + c * g.n + i3] = make_double2(xv.x - q.x, xv.y - q.y);
+        }
+    }
+}
+
 __global__ void chat64_layout_kernel(const cplx* __restrict__ chat, cplx* __restrict__ chat64) {
     const long total = 64L * 64 * 64;
     for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
@@ -180,8 +309,23 @@ cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cpl
     xy_conv64_kernel<<<dim3(64, 3, batch), 256, XY64_SMEM, st>>>(g, d_W, d_chat64, d_active);
     return cudaGetLastError();
 }
+static const size_t ZI64_SMEM = sizeof(cplx) * (2 * 64 * 32 + 32 * SC_LINE);
+cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const int* d_active,
+                               cudaStream_t st) {
+    z_forward64_kernel<<<dim3((g.NL + 31) / 32, 3, batch), 256, XY64_SMEM, st>>>(g, d_x, d_W, d_active);
+    return cudaGetLastError();
+}
+cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* d_W, const cplx* d_x, cplx* d_y,
+                                     const double* d_kvec, const double* d_k0, const int* d_active, cudaStream_t st) {
+    z_inverse_green64_kernel<<<dim3((g.NL + 31) / 32, batch), 256, ZI64_SMEM, st>>>(g, d_W, d_x, d_y, d_kvec, d_k0,
+                                                                                     d_active);
+    return cudaGetLastError();
+}
 cudaError_t apply64_init_attributes() {
-    return cudaFuncSetAttribute(xy_conv64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(xy_conv64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZI64_SMEM);
+    return e;
 }
 
 }  // namespace gsm

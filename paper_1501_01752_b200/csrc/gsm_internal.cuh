@@ -76,6 +76,10 @@ cudaError_t apply_init_attributes();
 bool apply64_usable(const ApplyGeom& g);
 cudaError_t apply64_init_attributes();
 cudaError_t launch_chat64_layout(const cplx* d_chat, cplx* d_chat64, cudaStream_t st);
+cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const int* d_active,
+                               cudaStream_t st);
+cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* d_W, const cplx* d_x, cplx* d_y,
+                                     const double* d_kvec, const double* d_k0, const int* d_active, cudaStream_t st);
 cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat64, const int* d_active,
                              cudaStream_t st);
 cudaError_t plan_init_attributes();
