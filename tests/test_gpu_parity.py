@@ -101,6 +101,14 @@ def test_apply_anisotropic_orders():
     _apply_case(geo, 2, 7, orc.toeplitz_matvec_c)
 
 
+@pytest.mark.parametrize("orders", [(17, 32, 25), (32, 32, 32), (20, 31, 17), (31, 17, 32)])
+def test_apply_64_point_axes_ragged(orders):
+    """All three axes on the 64-point fast path (apply64.cu) with every padding/pruning predicate exercised:
+    17..32 harmonics per axis, even and odd counts, line counts that are not multiples of the 32-line tiles."""
+    geo = wl.Geometry("p64", (0.2, 0.25, 0.3), orders, wl.ellipsoid_lattice().shapes, 1.0, 1.1 + 0.05j, None, ())
+    _apply_case(geo, 2, 13, orc.toeplitz_matvec_c)
+
+
 def test_apply_unit_vector_returns_column():
     # x = e_(c, m') -> (T x)_m = c_{m-m'}; with k0 -> G known, check through the oracle's Green multiply
     geo = wl.sphere_lattice((7, 7, 7))
