@@ -107,12 +107,14 @@ static __device__ __forceinline__ cplx cluster_sum(MgsSmem* sm, cplx v, int step
     return q[0];
 }
 
-// grid = batch * CS CTAs, cluster = CS CTAs along x; chunk = elements per CTA (<= MGS_T * MGS_E).
+// Persistent: grid = nclusters * CS CTAs (cluster = CS CTAs along x); cluster k runs solves k, k + nclusters, ...
+// chunk = elements per CTA (<= MGS_T * MGS_E).  The first two basis slices of the NEXT solve are requested as soon as
+// the last slice of the current one has been used, so the norm exchange, the write of v_{j+1}, the Givens update and
+// the load of the next w all run under that transfer.
 __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, KrylovState s, int batch, int j, int chunk) {
     cg::cluster_group cluster = cg::this_cluster();
     const unsigned cs = cluster.num_blocks(), rank = cluster.block_rank();
-    const int b = blockIdx.x / cs;
-    if (!s.active[b]) return;   // uniform over the cluster: the flag only changes at the very end of this kernel
+    const int nclusters = gridDim.x / cs;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx* vbuf0 = reinterpret_cast<cplx*>(smem_raw);
@@ -127,8 +129,6 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     const int len = (int)max(0L, min((long)chunk, d.vlen - lo));
     const uint32_t bytes = (uint32_t)len * (uint32_t)sizeof(cplx);
     const long vs = (long)batch * d.vlen;
-    const cplx* vb = s.basis + (long)b * d.vlen + lo;            // slice of v_0; v_i at + i * vs
-    cplx* wg = s.basis + (long)b * d.vlen + (long)(j + 1) * vs + lo;
 
     if (t == 0) {
         mbar_init(&sm->mbar[0], 1);
@@ -138,75 +138,95 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (t == 0 && len > 0) {
+    // solves of this cluster that are still iterating (only this cluster ever changes their flags)
+    auto next_active = [&](int from) {
+        while (from < batch && !s.active[from]) from += nclusters;
+        return from;
+    };
+    auto prefetch_first_two = [&](int bb) {   // thread 0 only
+        const cplx* vb = s.basis + (long)bb * d.vlen + lo;
         mbar_expect_tx(&sm->mbar[0], bytes);
         bulk_g2s(vbuf0, vb, bytes, &sm->mbar[0]);
         if (j >= 1) {
             mbar_expect_tx(&sm->mbar[1], bytes);
             bulk_g2s(vbuf1, vb + vs, bytes, &sm->mbar[1]);
         }
-    }
-    if (rank == 0)
-        for (int i = t; i < j; i += MGS_T) {
-            cssm[i] = s.cs[(long)b * d.mmax + i];
-            snsm[i] = s.sn[(long)b * d.mmax + i];
-        }
-    cplx w[MGS_E];
-#pragma unroll
-    for (int k = 0; k < MGS_E; ++k) {
-        const int e = k * MGS_T + t;
-        w[k] = (e < len) ? wg[e] : make_double2(0.0, 0.0);
-    }
+    };
+    int b = next_active((int)(blockIdx.x / cs));
+    if (t == 0 && len > 0 && b < batch) prefetch_first_two(b);
     // every CTA of the cluster must have started (mbarriers initialised) before any remote write reaches it
     cluster.sync();
 
     uint32_t phase0 = 0, phase1 = 0;
-    for (int i = 0; i <= j; ++i) {
-        cplx* vbuf = (i & 1) ? vbuf1 : vbuf0;
-        if (len > 0) {
-            if (i & 1) { mbar_wait(&sm->mbar[1], phase1); phase1 ^= 1; }
-            else       { mbar_wait(&sm->mbar[0], phase0); phase0 ^= 1; }
-        }
-        cplx acc = make_double2(0.0, 0.0);
+    int xstep = 0;   // running exchange number of cluster_sum
+    while (b < batch) {
+        const cplx* vb = s.basis + (long)b * d.vlen + lo;            // slice of v_0; v_i at + i * vs
+        cplx* wg = s.basis + (long)b * d.vlen + (long)(j + 1) * vs + lo;
+        if (rank == 0)
+            for (int i = t; i < j; i += MGS_T) {
+                cssm[i] = s.cs[(long)b * d.mmax + i];
+                snsm[i] = s.sn[(long)b * d.mmax + i];
+            }
+        cplx w[MGS_E];
 #pragma unroll
-        for (int k = 0; k < MGS_E; ++k) {   // conj(v) * w
+        for (int k = 0; k < MGS_E; ++k) {
             const int e = k * MGS_T + t;
-            if (e < len) {
-                const cplx v = vbuf[e];
-                acc.x = fma(v.x, w[k].x, fma(v.y, w[k].y, acc.x));
-                acc.y = fma(v.x, w[k].y, fma(-v.y, w[k].x, acc.y));
+            w[k] = (e < len) ? wg[e] : make_double2(0.0, 0.0);
+        }
+        const int bnext = next_active(b + nclusters);
+        for (int i = 0; i <= j; ++i) {
+            cplx* vbuf = (i & 1) ? vbuf1 : vbuf0;
+            if (len > 0) {
+                if (i & 1) { mbar_wait(&sm->mbar[1], phase1); phase1 ^= 1; }
+                else       { mbar_wait(&sm->mbar[0], phase0); phase0 ^= 1; }
+            }
+            cplx acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int k = 0; k < MGS_E; ++k) {   // conj(v) * w
+                const int e = k * MGS_T + t;
+                if (e < len) {
+                    const cplx v = vbuf[e];
+                    acc.x = fma(v.x, w[k].x, fma(v.y, w[k].y, acc.x));
+                    acc.y = fma(v.x, w[k].y, fma(-v.y, w[k].x, acc.y));
+                }
+            }
+            const cplx h = cluster_sum(sm, acc, xstep++, cs, rank);
+#pragma unroll
+            for (int k = 0; k < MGS_E; ++k) {   // w -= h v
+                const int e = k * MGS_T + t;
+                if (e < len) {
+                    const cplx v = vbuf[e];
+                    w[k].x = fma(-h.x, v.x, fma(h.y, v.y, w[k].x));
+                    w[k].y = fma(-h.x, v.y, fma(-h.y, v.x, w[k].y));
+                }
+            }
+            if (t == 0) hsm[i] = h;
+            __syncthreads();   // every thread is done with vbuf: it may be refilled
+            if (t == 0 && len > 0) {
+                if (i + 2 <= j) {
+                    uint64_t* bar = &sm->mbar[i & 1];
+                    mbar_expect_tx(bar, bytes);
+                    bulk_g2s(vbuf, vb + (long)(i + 2) * vs, bytes, bar);
+                } else if (i == j && bnext < batch) {
+                    prefetch_first_two(bnext);   // both buffers are idle now
+                }
             }
         }
-        const cplx h = cluster_sum(sm, acc, i, cs, rank);
+        cplx nn = make_double2(0.0, 0.0);
 #pragma unroll
-        for (int k = 0; k < MGS_E; ++k) {   // w -= h v
+        for (int k = 0; k < MGS_E; ++k) nn.x = fma(w[k].x, w[k].x, fma(w[k].y, w[k].y, nn.x));
+        nn = cluster_sum(sm, nn, xstep++, cs, rank);
+        const double hn = sqrt(nn.x);
+        const double sc = hn > 0.0 ? 1.0 / hn : 0.0;
+#pragma unroll
+        for (int k = 0; k < MGS_E; ++k) {
             const int e = k * MGS_T + t;
-            if (e < len) {
-                const cplx v = vbuf[e];
-                w[k].x = fma(-h.x, v.x, fma(h.y, v.y, w[k].x));
-                w[k].y = fma(-h.x, v.y, fma(-h.y, v.x, w[k].y));
-            }
+            if (e < len) wg[e] = make_double2(w[k].x * sc, w[k].y * sc);
         }
-        if (t == 0) hsm[i] = h;
-        __syncthreads();   // every thread is done with vbuf: it may be refilled
-        if (t == 0 && len > 0 && i + 2 <= j) {
-            uint64_t* bar = &sm->mbar[i & 1];
-            mbar_expect_tx(bar, bytes);
-            bulk_g2s(vbuf, vb + (long)(i + 2) * vs, bytes, bar);
-        }
+        if (rank == 0 && t == 0) givens_step(d, s, b, j, hsm, hn, cssm, snsm);
+        __syncthreads();   // hsm / cssm / snsm are reused by the next solve
+        b = bnext;
     }
-    cplx nn = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int k = 0; k < MGS_E; ++k) nn.x = fma(w[k].x, w[k].x, fma(w[k].y, w[k].y, nn.x));
-    nn = cluster_sum(sm, nn, j + 1, cs, rank);
-    const double hn = sqrt(nn.x);
-    const double sc = hn > 0.0 ? 1.0 / hn : 0.0;
-#pragma unroll
-    for (int k = 0; k < MGS_E; ++k) {
-        const int e = k * MGS_T + t;
-        if (e < len) wg[e] = make_double2(w[k].x * sc, w[k].y * sc);
-    }
-    if (rank == 0 && t == 0) givens_step(d, s, b, j, hsm, hn, cssm, snsm);
     cluster.sync();   // no CTA leaves while a peer's asynchronous store to it could still be in flight
 }
 
@@ -217,7 +237,8 @@ size_t arnoldi_cluster_smem(const KrylovDims& d, int chunk) {
 
 // Smallest power-of-two cluster whose CTAs can each keep their slice of w in registers; 0 if the vector is too long
 // or the device cannot co-schedule such a cluster (then krylov.cu's two-sweep path is used).
-cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out) {
+cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out, int* nclusters_out) {
+    *nclusters_out = 0;
     *cs_out = 0;
     *chunk_out = 0;
     const long cap = (long)MGS_T * MGS_E;
@@ -249,14 +270,15 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     if (e != cudaSuccess || nclusters < 1) { cudaGetLastError(); return cudaSuccess; }
     *cs_out = cs;
     *chunk_out = chunk;
+    *nclusters_out = nclusters;
     return cudaSuccess;
 }
 
 cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
-                                   cudaStream_t st, Profiler* prof, int nact) {
+                                   int nclusters, cudaStream_t st, Profiler* prof, int nact) {
     ProfScope ps_(prof, KC_ARNOLDI_MGS, st, 16.0 * d.vlen * (j + 3.0) * nact);   // reads w, v_0..v_j; writes v_{j+1}
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)batch * cs);
+    cfg.gridDim = dim3((unsigned)(batch < nclusters ? batch : nclusters) * cs);
     cfg.blockDim = dim3(MGS_T);
     cfg.dynamicSmemBytes = arnoldi_cluster_smem(d, chunk);
     cfg.stream = st;

@@ -20,7 +20,7 @@ struct gsm_plan {
     cudaStream_t stream = nullptr;
     int max_batch = 1, max_iters = 64;
     long i0 = 0;                  // flat index of m = 0 inside one component
-    int mgs_cs = 0, mgs_chunk = 0; // cluster MGS Arnoldi step (0 = two-sweep fallback)
+    int mgs_cs = 0, mgs_chunk = 0, mgs_nclusters = 0; // cluster MGS Arnoldi step (0 = two-sweep fallback)
     std::vector<void*> allocs;    // every device allocation, freed in destroy
     long long device_bytes = 0;
     Profiler prof;
@@ -275,7 +275,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         kd.mmax = m;
         kd.ld = m + 1;
         KrylovState& ks = plan->ks;
-        CK(arnoldi_cluster_plan(kd, &plan->mgs_cs, &plan->mgs_chunk));
+        CK(arnoldi_cluster_plan(kd, &plan->mgs_cs, &plan->mgs_chunk, &plan->mgs_nclusters));
         if (getenv("GSM_FORCE_TWO_SWEEP")) plan->mgs_cs = 0;
         CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
         CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
@@ -415,7 +415,7 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
         CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
                         plan->W, ks.active, st, prof, nact));
         if (plan->mgs_cs > 0) {
-            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, st, prof, nact));
+            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, st, prof, nact));
         } else {
             CK(launch_sweep_dots(kd, ks, nb, j, st, prof, nact));
             CK(launch_hsolve(kd, ks, nb, j, st, prof));

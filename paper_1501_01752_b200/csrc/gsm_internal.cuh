@@ -137,8 +137,8 @@ cudaError_t krylov_init_attributes();
 // ---- launches implemented in arnoldi_cluster.cu ------------------------------------------------------------------
 // One Arnoldi step (MGS + norm + normalise + Givens) per solve in one thread-block cluster, basis read once.
 // arnoldi_cluster_plan: cluster size (0 = not usable: fall back to the two-sweep kernels) and elements per CTA.
-cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out);
+cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out, int* nclusters_out);
 cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
-                                   cudaStream_t st, Profiler* prof, int nact);
+                                   int nclusters, cudaStream_t st, Profiler* prof, int nact);
 
 }  // namespace gsm
