@@ -172,18 +172,31 @@ size_t apply_smem_max(const ApplyGeom& g) {
 cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
                          cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact) {
     const int nlt = (g.NL + g.L - 1) / g.L;
-    // algorithmic bytes of the three passes as designed: field vector V = 3n, z-transformed intermediate 3 P3 NL
-    const double V = 16.0 * 3.0 * g.n * nact, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL * nact;
+    // The batch can go through the three passes `sub` solves at a time through the SAME workspace W (stream order
+    // keeps sub-batches apart), which keeps W in L2; measured slower than one pass at 31^3 (see gsm_api.cu), so
+    // sub == batch unless GSM_APPLY_SUB is set.
+    const int sub = g.sub > 0 ? g.sub : batch;
     const double Cb = 16.0 * g.ax[0].P * g.ax[1].P * g.ax[2].P;
-    { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
-      if (g.chat64) launch_z_forward64(g, batch, d_x, d_W, d_active, st);
-      else z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_active); }
-    { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
-      if (g.chat64) launch_xy_conv64(g, batch, d_W, g.chat64, d_active, st);
-      else xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); }
-    { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
-      if (g.chat64) launch_z_inverse_green64(g, batch, d_W, d_x, d_y, d_kvec, d_k0, d_active, st);
-      else z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); }
+    for (int b0 = 0; b0 < batch; b0 += sub) {
+        const int nb = batch - b0 < sub ? batch - b0 : sub;
+        const double frac = (double)nact * nb / batch;
+        // algorithmic bytes of the three passes as designed: field vector V = 3n, z-transformed intermediate 3 P3 NL
+        const double V = 16.0 * 3.0 * g.n * frac, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL * frac;
+        const cplx* x = d_x + (long)b0 * 3 * g.n;
+        cplx* y = d_y + (long)b0 * 3 * g.n;
+        const double* kv = d_kvec + 3 * b0;
+        const double* k0 = d_k0 + b0;
+        const int* act = d_active ? d_active + b0 : nullptr;
+        { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
+          if (g.chat64) launch_z_forward64(g, nb, x, d_W, act, st);
+          else z_forward_kernel<<<dim3(nlt, 3, nb), 256, smem_pass1(g), st>>>(g, x, d_W, act); }
+        { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
+          if (g.chat64) launch_xy_conv64(g, nb, d_W, g.chat64, act, st);
+          else xy_conv_kernel<<<dim3(g.ax[2].P, 3, nb), 256, smem_pass2(g), st>>>(g, d_W, act); }
+        { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
+          if (g.chat64) launch_z_inverse_green64(g, nb, d_W, x, y, kv, k0, act, st);
+          else z_inverse_green_kernel<<<dim3(nlt, nb), 256, smem_pass3(g), st>>>(g, d_W, x, y, kv, k0, act); }
+    }
     return cudaGetLastError();
 }
 

@@ -277,7 +277,13 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         KrylovState& ks = plan->ks;
         CK(arnoldi_cluster_plan(kd, &plan->mgs_cs, &plan->mgs_chunk, &plan->mgs_nclusters));
         if (getenv("GSM_FORCE_TWO_SWEEP")) plan->mgs_cs = 0;
-        CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
+        {   // Sub-batching the apply so that W stays in L2 was measured and LOSES at 31^3 (sub = 8/16/32: step 208/185/
+            // 173 ms vs 157 ms for the whole batch: short kernels pay launch gaps and tails), so the default is one pass.
+            int sub = B;
+            if (const char* e = getenv("GSM_APPLY_SUB")) sub = atoi(e);
+            g.sub = std::max(1, std::min(B, sub));
+        }
+        CK(dalloc(plan, &plan->W, (size_t)g.sub * 3 * g.ax[2].P * g.NL));
         CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &plan->ybuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &ks.basis, (size_t)kd.ld * B * kd.vlen));

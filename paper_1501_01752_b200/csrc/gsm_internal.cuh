@@ -44,6 +44,7 @@ struct ApplyGeom {
     int N1, N2, N3;      // harmonics kept
     int NL;              // N1*N2 = number of z-lines per component
     long n;              // N1*N2*N3
+    int sub;             // solves per pass through the workspace W (L2-resident sub-batches)
     int L;               // z-lines per CTA in passes 1 and 3
     int Lst;             // odd row stride (>= L) of the pass-1 tile
     int RS3;             // odd row stride (>= 3L) of the pass-3 tile
