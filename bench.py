@@ -52,13 +52,15 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def _traffic(kernel):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/ncu_traffic.json)."""
+def _traffic(kernel, alg_bytes_per_launch):
+    """DRAM bytes per launch of `kernel`: the dram/algorithmic ratio of the committed ncu --set full capture
+    (profiles/ncu_traffic.json) scaled to the average launch of the timed region; None if that kernel was not captured."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
     if not os.path.exists(path):
         return None
     with open(path) as f:
-        return json.load(f).get(kernel, {}).get("dram_bytes_per_launch")
+        ratio = json.load(f).get(kernel, {}).get("ratio")
+    return None if ratio is None else ratio * alg_bytes_per_launch
 
 
 class ClockSampler:
@@ -290,7 +292,7 @@ def run_gsm(args):
         "gpu_launches": gpu_launches,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": _traffic(dom), "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": _traffic(dom, by_l / n_l), "peak_source": peak_src,
                      "launches": n_l, "avg_launch_ms": ms_l / n_l, "algorithmic_bytes_per_launch": by_l / n_l,
                      "share_of_step": ms_l / kernels_ms},
         "path_roofline": {"algorithmic_GBps": path_gbs, "frac": path_gbs / peak,
