@@ -4,11 +4,12 @@
 //   for i = 0..j:  h_i = <v_i, w>;  w <- w - h_i v_i          (Saad Alg. 6.9, lines 4-7)
 //   h_{j+1,j} = ||w||;  v_{j+1} = w / h_{j+1,j}               (lines 8-9), then the Givens update of the least squares
 //
-// One solve = one thread-block cluster.  The cluster keeps w on chip (registers, vlen / (CS * 512) complex numbers
+// One solve = one thread-block cluster.  The cluster keeps w on chip (registers, vlen / (CS * 256) complex numbers
 // per thread) for the whole step.  Each v_i is streamed through shared memory exactly once: a 1-D bulk TMA copy
 // (cp.async.bulk + mbarrier) brings CTA r's contiguous slice of v_i into one of two buffers while the previous
 // slice is being used, the slice is dotted with w, the partial sums are exchanged through distributed shared memory
-// (st.async + mbarrier, no cluster-wide barrier), and the same slice - still in shared memory - updates w.  HBM traffic per step is
+// (st.async + mbarrier, no cluster-wide barrier), and the same slice - read from shared memory once and held in
+// registers across the exchange, so its buffer is refilled while the sums travel - updates w.  HBM traffic per step is
 // (j + 3) V: read w, read v_0..v_j, write v_{j+1}; the paper's one-CUBLAS-call-per-dot/axpy schedule (made for a
 // GTX Titan) moves 5 V per basis vector, the two-sweep fallback in krylov.cu 2 V.
 //
@@ -23,8 +24,8 @@ namespace cg = cooperative_groups;
 
 namespace gsm {
 
-#define MGS_T 512        // threads per CTA
-#define MGS_E 11         // complex elements of w per thread (registers)
+#define MGS_T 256        // threads per CTA
+#define MGS_E 22         // complex elements of w per thread (registers)
 #define MGS_MAXCS 16     // largest cluster (non-portable size, opt-in)
 #define MGS_NW (MGS_T / 32)
 
@@ -81,7 +82,7 @@ struct MgsSmem {
 // can only send exchange s+2 after it has received every rank's exchange s+1, which rank Y sends after all of its
 // threads have consumed exchange s - so two pairs never collide.  All ranks sum the same values in the same fixed
 // tree order: identical bits everywhere, deterministic.
-static __device__ __forceinline__ cplx cluster_sum(MgsSmem* sm, cplx v, int step, unsigned cs, unsigned rank) {
+static __device__ __forceinline__ void cluster_sum_send(MgsSmem* sm, cplx v, int step, unsigned cs, unsigned rank) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, par = step & 1;
     v.x = warp_sum_x(v.x);
     v.y = warp_sum_x(v.y);
@@ -96,6 +97,9 @@ static __device__ __forceinline__ cplx cluster_sum(MgsSmem* sm, cplx v, int step
         if (lane < (int)cs)
             st_async_cplx(map_rank(smem_u32(&sm->red[par][rank]), lane), t, map_rank(smem_u32(&sm->rbar[par]), lane));
     }
+}
+static __device__ __forceinline__ cplx cluster_sum_recv(MgsSmem* sm, int step, unsigned cs) {
+    const int par = step & 1;
     mbar_wait(&sm->rbar[par], (step >> 1) & 1);
     cplx q[MGS_MAXCS];
 #pragma unroll
@@ -181,28 +185,16 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
                 else       { mbar_wait(&sm->mbar[0], phase0); phase0 ^= 1; }
             }
             cplx acc = make_double2(0.0, 0.0);
+            cplx v[MGS_E];   // the slice is read from shared memory once and kept for the update
 #pragma unroll
             for (int k = 0; k < MGS_E; ++k) {   // conj(v) * w
                 const int e = k * MGS_T + t;
-                if (e < len) {
-                    const cplx v = vbuf[e];
-                    acc.x = fma(v.x, w[k].x, fma(v.y, w[k].y, acc.x));
-                    acc.y = fma(v.x, w[k].y, fma(-v.y, w[k].x, acc.y));
-                }
+                v[k] = (e < len) ? vbuf[e] : make_double2(0.0, 0.0);
+                acc.x = fma(v[k].x, w[k].x, fma(v[k].y, w[k].y, acc.x));
+                acc.y = fma(v[k].x, w[k].y, fma(-v[k].y, w[k].x, acc.y));
             }
-            const cplx h = cluster_sum(sm, acc, xstep++, cs, rank);
-#pragma unroll
-            for (int k = 0; k < MGS_E; ++k) {   // w -= h v
-                const int e = k * MGS_T + t;
-                if (e < len) {
-                    const cplx v = vbuf[e];
-                    w[k].x = fma(-h.x, v.x, fma(h.y, v.y, w[k].x));
-                    w[k].y = fma(-h.x, v.y, fma(-h.y, v.x, w[k].y));
-                }
-            }
-            if (t == 0) hsm[i] = h;
-            __syncthreads();   // every thread is done with vbuf: it may be refilled
-            if (t == 0 && len > 0) {
+            cluster_sum_send(sm, acc, xstep, cs, rank);   // contains a block barrier: every thread has read vbuf
+            if (t == 32 && len > 0) {                     // so the buffer can be refilled while the sums travel
                 if (i + 2 <= j) {
                     uint64_t* bar = &sm->mbar[i & 1];
                     mbar_expect_tx(bar, bytes);
@@ -211,11 +203,19 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
                     prefetch_first_two(bnext);   // both buffers are idle now
                 }
             }
+            const cplx h = cluster_sum_recv(sm, xstep++, cs);
+#pragma unroll
+            for (int k = 0; k < MGS_E; ++k) {   // w -= h v
+                w[k].x = fma(-h.x, v[k].x, fma(h.y, v[k].y, w[k].x));
+                w[k].y = fma(-h.x, v[k].y, fma(-h.y, v[k].x, w[k].y));
+            }
+            if (t == 0) hsm[i] = h;
         }
         cplx nn = make_double2(0.0, 0.0);
 #pragma unroll
         for (int k = 0; k < MGS_E; ++k) nn.x = fma(w[k].x, w[k].x, fma(w[k].y, w[k].y, nn.x));
-        nn = cluster_sum(sm, nn, xstep++, cs, rank);
+        cluster_sum_send(sm, nn, xstep, cs, rank);
+        nn = cluster_sum_recv(sm, xstep++, cs);
         const double hn = sqrt(nn.x);
         const double sc = hn > 0.0 ? 1.0 / hn : 0.0;
 #pragma unroll
