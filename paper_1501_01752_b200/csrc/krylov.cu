@@ -98,24 +98,31 @@ __global__ void __launch_bounds__(KT) sweep_dots_kernel(KrylovDims d, KrylovStat
 }
 
 // per solve: reduce the partials, store the Gram row, run the MGS recurrence -> hcol[0..j]
-__global__ void __launch_bounds__(32) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+// HS_T threads: warp w reduces the partials of entries i = w, w + HS_T/32, ... (lanes stride over the chunks, fixed
+// shuffle tree: deterministic), then warp 0 runs the recurrence.
+#define HS_T 256
+__global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j) {
     const int b = blockIdx.x;
     if (!s.active[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* dd = reinterpret_cast<cplx*>(smem_raw);   // [ld]
     cplx* gT = s.gram + (long)b * d.ld * d.ld;      // gT[k*ld + i] = <v_k, v_i>, k <= i
-    const int lane = threadIdx.x;
-    for (int i = lane; i <= j; i += 32) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = warp; i <= j; i += HS_T / 32) {
         double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
         const cplx* p = s.part + (long)b * d.nchunk * 2 * d.ld + 2 * i;
-        for (int c = 0; c < d.nchunk; ++c) {
+        for (int c = lane; c < d.nchunk; c += 32) {
             const cplx a = p[(long)c * 2 * d.ld], g = p[(long)c * 2 * d.ld + 1];
             a0 += a.x; a1 += a.y; g0 += g.x; g1 += g.y;
         }
-        dd[i] = make_double2(a0, a1);
-        gT[(long)i * d.ld + j] = make_double2(g0, g1);
+        a0 = warp_sum(a0); a1 = warp_sum(a1); g0 = warp_sum(g0); g1 = warp_sum(g1);
+        if (lane == 0) {
+            dd[i] = make_double2(a0, a1);
+            gT[(long)i * d.ld + j] = make_double2(g0, g1);
+        }
     }
-    __syncwarp();
+    __syncthreads();
+    if (warp != 0) return;
     // column-oriented recurrence: once h_k is final, every later d_i loses h_k <v_i, v_k> = h_k conj(<v_k, v_i>)
     for (int k = 0; k < j; ++k) {
         const cplx hk = dd[k];
@@ -180,11 +187,13 @@ __global__ void __launch_bounds__(KT) sweep_update_kernel(KrylovDims d, KrylovSt
 }
 
 // two-sweep path: h_{j+1,j} = ||w|| from the partial norms of sweep 2, then the Givens step
-__global__ void givens_kernel(KrylovDims d, KrylovState s, int batch, int j) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= batch || !s.active[b]) return;
+__global__ void givens_kernel(KrylovDims d, KrylovState s, int batch, int j) {   // one warp per solve
+    const int b = blockIdx.x;
+    if (!s.active[b]) return;
     double nn = 0.0;
-    for (int c = 0; c < d.nchunk; ++c) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    for (int c = threadIdx.x; c < d.nchunk; c += 32) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    nn = warp_sum(nn);
+    if (threadIdx.x != 0) return;
     givens_step(d, s, b, j, s.hcol + (long)b * d.ld, sqrt(nn), s.cs + (long)b * d.mmax, s.sn + (long)b * d.mmax);
 }
 
@@ -309,7 +318,7 @@ cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int bat
 }
 cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
     ProfScope ps_(prof, KC_HSOLVE, st);
-    hsolve_kernel<<<batch, 32, sizeof(cplx) * d.ld, st>>>(d, s, batch, j);
+    hsolve_kernel<<<batch, HS_T, sizeof(cplx) * d.ld, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
 cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
@@ -319,7 +328,7 @@ cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int b
 }
 cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
     ProfScope ps_(prof, KC_GIVENS, st);
-    givens_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch, j);
+    givens_kernel<<<batch, 32, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
 cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
