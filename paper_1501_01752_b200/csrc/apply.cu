@@ -192,6 +192,7 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
           else z_forward_kernel<<<dim3(nlt, 3, nb), 256, smem_pass1(g), st>>>(g, x, d_W, act); }
         { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
           if (g.chat64) launch_xy_conv64(g, nb, d_W, g.chat64, act, st);
+          else if (g.chat128) launch_xy_conv128(g, nb, d_W, g.chat128, act, st);
           else xy_conv_kernel<<<dim3(g.ax[2].P, 3, nb), 256, smem_pass2(g), st>>>(g, d_W, act); }
         { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
           if (g.chat64) launch_z_inverse_green64(g, nb, d_W, x, y, kv, k0, act, st);
@@ -208,6 +209,7 @@ cudaError_t apply_init_attributes() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(xy_conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = apply64_init_attributes();
+    if (e == cudaSuccess) e = apply128_init_attributes();
     return e;
 }
 }  // namespace gsm

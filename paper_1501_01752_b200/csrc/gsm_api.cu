@@ -25,6 +25,8 @@ struct gsm_plan {
     long long device_bytes = 0;
     Profiler prof;
     cplx* chat64 = nullptr;
+    cplx* chat128 = nullptr;
+    int* gen128[2] = {nullptr, nullptr};
     cplx *coef = nullptr, *chat = nullptr, *pad = nullptr, *W = nullptr, *xbuf = nullptr, *ybuf = nullptr;
     size_t vgrid_count = 0;
     cplx* vgrid = nullptr;        // voxel path: device copy of the grid, transformed in place
@@ -214,6 +216,19 @@ static gsm_status build_spectrum(gsm_plan* plan) {
         if (!plan->chat64) CK(dalloc(plan, &plan->chat64, np));
         e = launch_chat64_layout(plan->chat, plan->chat64, plan->stream);
         g.chat64 = plan->chat64;
+    }
+    if (e == cudaSuccess && apply128_usable(g) && !getenv("GSM_GENERIC_APPLY")) {
+        if (!plan->chat128) {
+            CK(dalloc(plan, &plan->chat128, np));
+            for (int a = 0; a < 2; ++a) {   // new position -> frequency -> position in the generic network
+                std::vector<int> gen(128);
+                for (int q = 0; q < 128; ++q) gen[q] = pos_of_freq(apply128_freq_of_pos(q), 128, g.ax[a].radix, g.ax[a].nst);
+                CK(dalloc(plan, &plan->gen128[a], (size_t)128));
+                CK(cudaMemcpy(plan->gen128[a], gen.data(), sizeof(int) * 128, cudaMemcpyHostToDevice));
+            }
+        }
+        e = launch_chat128_layout(plan->chat, P[2], plan->gen128[0], plan->gen128[1], plan->chat128, plan->stream);
+        g.chat128 = plan->chat128;
     }
     CK(e);
     g.chat = plan->chat;

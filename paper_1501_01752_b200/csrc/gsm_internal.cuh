@@ -53,6 +53,7 @@ struct ApplyGeom {
     const cplx* tw[3];   // device twiddle tables exp(-2 pi i k / P_a)
     const cplx* chat;    // coefficient spectrum, position order, [P3][P1][P2], scaled by 1/(P1 P2 P3)
     const cplx* chat64;  // same, permuted for apply64.cu (null unless apply64_usable)
+    const cplx* chat128; // same, in the order of apply128.cu's x/y network (null unless apply128_usable)
     double K[3];         // 2 pi / Lambda_a
     int mmin[3];         // lowest order per axis
     double epsb_re, epsb_im;
@@ -73,6 +74,14 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
                          cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact);
 size_t apply_smem_max(const ApplyGeom& g);
 cudaError_t apply_init_attributes();
+// apply128.cu: pass 2 specialised for 128-point x and y axes
+bool apply128_usable(const ApplyGeom& g);
+int apply128_freq_of_pos(int p);
+cudaError_t apply128_init_attributes();
+cudaError_t launch_chat128_layout(const cplx* d_chat, int P3, const int* d_gen1, const int* d_gen2, cplx* d_chat128,
+                                  cudaStream_t st);
+cudaError_t launch_xy_conv128(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat128, const int* d_active,
+                              cudaStream_t st);
 // apply64.cu: passes specialised for 64-point axes (chat64 = Chat permuted for 8-lane groups)
 bool apply64_usable(const ApplyGeom& g);
 cudaError_t apply64_init_attributes();

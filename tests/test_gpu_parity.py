@@ -126,10 +126,15 @@ def test_apply_unit_vector_returns_column():
     plan.close()
 
 
-@pytest.mark.parametrize("orders,nsamp", [((31, 31, 31), 24), ((63, 63, 63), 6)])
+@pytest.mark.parametrize("orders,nsamp", [((31, 31, 31), 24), ((63, 63, 63), 6), ((33, 64, 40), 10), ((64, 40, 9), 10)])
 def test_apply_full_size_sampled_rows(orders, nsamp):
     """BASELINE sizes (configs 4/5): sampled output harmonics against the oracle's O(n) row sum."""
-    geo = wl.woodpile(orders) if orders[0] == 31 else wl.sphere_lattice(orders, period=0.25, radius_frac=0.15, eps=6.0)
+    if orders == (31, 31, 31):
+        geo = wl.woodpile(orders)
+    elif orders == (63, 63, 63):
+        geo = wl.sphere_lattice(orders, period=0.25, radius_frac=0.15, eps=6.0)
+    else:   # ragged / even counts on the 128-point xy fast path (apply128.cu), z axis on the generic network
+        geo = wl.Geometry("p128", (0.2, 0.25, 0.3), orders, wl.ellipsoid_lattice().shapes, 1.0, 1.1 + 0.05j, None, ())
     batch = 2
     plan = gsm.plan_from_geometry(geo, max_batch=batch)
     c = oracle_coeffs(geo)
@@ -140,7 +145,7 @@ def test_apply_full_size_sampled_rows(orders, nsamp):
     rng = np.random.default_rng(9)
     N = orders
     samples = [(0, 0, 0), (N[0] - 1, N[1] - 1, N[2] - 1), (N[0] // 2, N[1] // 2, N[2] // 2), (N[0] - 1, 0, N[2] // 2)]
-    samples += [tuple(int(v) for v in rng.integers(0, N[0], 3)) for _ in range(nsamp)]
+    samples += [tuple(int(rng.integers(0, N[a])) for a in range(3)) for _ in range(nsamp)]
     scale = np.sqrt(np.mean(np.abs(y) ** 2))
     for b in range(batch):
         k = orc.wavevectors(geo.periods, orders, kb[b])
