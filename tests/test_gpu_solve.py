@@ -171,3 +171,66 @@ def test_scan_mixed_convergence_and_repeatability():
     assert len(set(ia.tolist())) > 1
     assert np.array_equal(ia, ib) and np.array_equal(ra, rb)      # deterministic reductions: bit-identical
     pa.close(); pb.close()
+
+
+def test_config5a_bench_configuration_sampled_points():
+    """BASELINE config 5a exactly as bench.py times it (voxel composite, 31^3 orders, one lock-step batch of 256, the
+    64-point fast path and the cluster MGS kernel): every solve meets the residual bar; sampled points are compared
+    field by field with the oracle's own GMRES on the O(n^2) product."""
+    geo = wl.voxel_composite((31, 31, 31), nv=128)
+    kappa = wl.kappa_mesh(1.05, 1.20, 256)
+    kb, kk, pol = wl.scan_points(kappa, 2, 0)
+    plan = gsm.plan_from_geometry(geo, max_iters=64, max_batch=256)
+    fields = torch.empty((256, 3, 31, 31, 31), dtype=torch.complex128, device="cuda")
+    resp, iters, resid, st = plan.scan(kb, kk, pol, tol=1e-12, fields=fields)
+    assert st == gsm.OK and np.all(resid <= 1e-10)
+    assert iters.min() >= 10 and iters.max() <= 64                  # PAPER.md:103 band
+    c = coeffs(geo)
+    for p in (3, 201):
+        ref, _, oit = orc.solve_gmres(c, geo.periods, geo.orders, kb[p], TWO_PI, geo.eps_b, [1.0, 0, 0], tol=1e-13,
+                                      max_iters=100, matvec=orc.toeplitz_matvec_c)
+        assert rel(fields[p].cpu().numpy(), ref) <= 1e-9
+        assert abs(int(iters[p]) - oit) <= 5
+        assert abs(resp[p, 0] - orc.zero_order(ref)[0]) <= 1e-9 * abs(orc.zero_order(ref)[0])
+    # the response is the m = 0 entry of the returned field, for every point
+    F0 = fields[:, :, 15, 15, 15].cpu().numpy()
+    assert np.array_equal(F0, resp)
+    plan.close()
+
+
+def test_config3_eps_xx_retrieval_vs_oracle_pipeline():
+    """BASELINE config 3, tensor entry xx (k || z, a = x, reading R14): scan -> pole search -> eps_eff on both sides.
+    The kappa mesh is placed by the ORACLE's coarse scan (pole mid-way between two nodes, reading R16)."""
+    geo = wl.ellipsoid_lattice((15, 15, 15))
+    c = coeffs(geo)
+    k0 = TWO_PI
+
+    def oracle_xi(kap):
+        out = np.zeros(len(kap), dtype=complex)
+        for i, kv in enumerate(kap):
+            E, _, _ = orc.solve_gmres(c, geo.periods, geo.orders, np.array([0, 0, kv]), k0, geo.eps_b, [1.0, 0, 0],
+                                      tol=1e-13, max_iters=150, matvec=orc.toeplitz_matvec_c)
+            out[i] = orc.zero_order(E)[0]
+        return out
+    coarse = wl.kappa_mesh(1.02, 1.30, 29)
+    xc = oracle_xi(coarse)
+    eta_c, zeta_c = orc.pole_search(coarse, xc, 5, 10)
+    bc = orc.select_pole(eta_c, zeta_c, coarse[0], coarse[-1])
+    assert bc >= 0
+    step = 0.002 * k0
+    fine = eta_c[bc].real + step * (np.arange(18) - 8.5)          # estimate falls mid-way between two nodes
+    xi_o = oracle_xi(fine)
+    eta_o, zeta_o = orc.pole_search(fine, xi_o, 5, 10)
+    bo = orc.select_pole(eta_o, zeta_o, fine[0], fine[-1])
+    n_o, eps_o = orc.retrieve_eps(eta_o[bo], k0)
+
+    plan = gsm.plan_from_geometry(geo, max_iters=120, max_batch=18)
+    kb, kk, pol = wl.scan_points(fine, 2, 0)
+    resp, iters, resid, st = plan.scan(kb, kk, pol, tol=1e-12)
+    assert st == gsm.OK and np.all(resid <= 1e-10)
+    eta, zeta, best = gsm.pole_search(fine, resp[:, 0], 5, 10)
+    assert best >= 0
+    eps_g = (eta[best] / k0) ** 2
+    assert abs(eps_g - eps_o) <= 1e-8
+    assert abs(eps_o.real - 1.11151881 ** 2) <= 2e-6      # SURVEY 8(c) orientation value for (z, x) at 15^3
+    plan.close()
