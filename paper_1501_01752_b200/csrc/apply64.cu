@@ -26,7 +26,10 @@ namespace gsm {
 //   y inverse : mirror of y forward, stores straight to W
 // chat64 is Chat permuted so that the 8 lanes of a group read 8 consecutive coefficients:
 //   chat64[((pos3 * 64 + r) * 8 + q) * 8 + u] = Chat[pos3][pos1 = 8u + q][pos2 = r].
-__global__ void __launch_bounds__(256, 3) xy_conv64_kernel(ApplyGeom g, cplx* __restrict__ W,
+#ifndef XY64_MINB
+#define XY64_MINB 2   // measured: 2 CTAs/SM at 122 registers (no spills) beats 3 CTAs/SM at 80 (46 vs 52 ms)
+#endif
+__global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, cplx* __restrict__ W,
                                                            const cplx* __restrict__ chat64,
                                                            const int* __restrict__ active) {
     const int b = blockIdx.z, c = blockIdx.y, pos3 = blockIdx.x;
@@ -56,7 +59,11 @@ __global__ void __launch_bounds__(256, 3) xy_conv64_kernel(ApplyGeom g, cplx* __
     }
     __syncthreads();
     // ---- x: forward, multiply by the coefficient spectrum, inverse
+#ifdef XY64_UNROLL
+#pragma unroll
+#else
 #pragma unroll 1
+#endif
     for (int round = 0; round < 2; ++round) {
         const int r = (round * 8 + warp) * 4 + ln;
         cplx* Ar = A + r * 32;
@@ -66,10 +73,19 @@ __global__ void __launch_bounds__(256, 3) xy_conv64_kernel(ApplyGeom g, cplx* __
             const int i1 = u + 8 * p;
             a[p] = (i1 < N1) ? Ar[(i1 + rot) & 31] : make_double2(0.0, 0.0);
         }
-        fwd64_group(a, tw, sc, u);
         const cplx* cp = chat64 + ((long)(pos3 * 64 + r) * 64) + u;
+#ifdef XY64_PREFETCH
+        cplx ch[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) ch[q] = __ldg(cp + 8 * q);
+        fwd64_group(a, tw, sc, u);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], ch[q]);
+#else
+        fwd64_group(a, tw, sc, u);
 #pragma unroll
         for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], __ldg(cp + 8 * q));
+#endif
         inv64_group(a, tw, sc, u);
 #pragma unroll
         for (int p = 0; p < 4; ++p) {

@@ -234,3 +234,26 @@ def test_config3_eps_xx_retrieval_vs_oracle_pipeline():
     assert abs(eps_g - eps_o) <= 1e-8
     assert abs(eps_o.real - 1.11151881 ** 2) <= 2e-6      # SURVEY 8(c) orientation value for (z, x) at 15^3
     plan.close()
+
+
+def test_degenerate_inputs_empty_scan_zero_source_and_largest_orders():
+    geo = wl.sphere_lattice((5, 5, 5))
+    plan = gsm.plan_from_geometry(geo, max_batch=4)
+    resp, iters, resid, st = plan.scan(np.zeros((0, 3)), np.zeros(0), np.zeros((0, 6)), tol=1e-10)
+    assert st == gsm.OK and resp.shape == (0, 3) and len(iters) == 0
+    # zero source: b = 0 -> E = 0 without iterating; mixed with a normal point in the same batch
+    kb = np.array([[0, 0, 1.2 * TWO_PI], [0, 0, 1.2 * TWO_PI]])
+    pol = np.zeros((2, 6)); pol[1, 0] = 1.0
+    fields = torch.full((2, 3, 5, 5, 5), 7.0, dtype=torch.complex128, device="cuda")
+    resp, iters, resid, st = plan.scan(kb, np.full(2, TWO_PI), pol, tol=1e-11, fields=fields)
+    assert st == gsm.OK and iters[0] == 0 and iters[1] > 3 and resid[0] == 0.0 and resid[1] <= 1e-10
+    assert float(fields[0].abs().max()) == 0.0 and np.all(resp[0] == 0)
+    plan.close()
+    # largest supported order count per axis (64 -> 128-point axis) and its neighbour are accepted; 65 is rejected
+    big = wl.Geometry("max", (0.2, 0.2, 0.2), (64, 1, 2), geo.shapes, 1.0, 1.0, None, ())
+    p2 = gsm.plan_from_geometry(big)
+    assert p2.info()["fft_grid"] == (128, 1, 4)
+    p2.close()
+    with pytest.raises(gsm.GsmError) as e:
+        gsm.Plan((0.2, 0.2, 0.2), (65, 1, 1), shapes=geo.shapes)
+    assert e.value.status == gsm.E_INVALID
