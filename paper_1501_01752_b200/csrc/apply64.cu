@@ -112,13 +112,16 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
 // CTA = 32 consecutive z-lines of one (b, c).  Each group loads its line's <= 32 inputs straight from x (contiguous),
 // transforms, and drops the 64 outputs into a [pos3][32 lines] tile (columns rotated by pos3/8: conflict-free), which
 // is then written to W[b][c][pos3][l] as 512-byte rows.
-__global__ void __launch_bounds__(256, 3) z_forward64_kernel(ApplyGeom g, const cplx* __restrict__ x, cplx* __restrict__ W,
-                                                             const int* __restrict__ active) {
+#ifndef ZF64_MINB
+#define ZF64_MINB 4
+#endif
+__global__ void __launch_bounds__(256, ZF64_MINB) z_forward64_kernel(ApplyGeom g, const cplx* __restrict__ x,
+                                                                     cplx* __restrict__ W, const int* __restrict__ active) {
     const int b = blockIdx.z, c = blockIdx.y;
     if (active && !active[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* T = reinterpret_cast<cplx*>(smem_raw);   // [64][32]
-    cplx* scratch = T + 64 * 32;
+    cplx* T = reinterpret_cast<cplx*>(smem_raw);   // [64][32] tile, aliases the scratch lines (barrier in between)
+    cplx* scratch = T;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, u = lane & 7, ln = lane >> 3;
     const int N3 = g.N3, NL = g.NL;
     cplx tw[7];
@@ -133,6 +136,7 @@ __global__ void __launch_bounds__(256, 3) z_forward64_kernel(ApplyGeom g, const 
         a[p] = (l < NL && i3 < N3) ? xs[i3] : make_double2(0.0, 0.0);
     }
     fwd64_group(a, tw, sc, u);
+    __syncthreads();   // every warp is done with its scratch lines: the tile may overwrite them
     const int col = (line + u) & 31;
 #pragma unroll
     for (int q = 0; q < 8; ++q) T[(8 * u + q) * 32 + col] = a[q];
@@ -259,10 +263,11 @@ cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cpl
     xy_conv64_kernel<<<dim3(64, 3, batch), 256, XY64_SMEM, st>>>(g, d_W, d_chat64, d_active);
     return cudaGetLastError();
 }
+static const size_t ZF64_SMEM = sizeof(cplx) * (32 * SC_LINE);   // >= 64 * 32 tile
 static const size_t ZI64_SMEM = sizeof(cplx) * (2 * 64 * 32 + 32 * SC_LINE);
 cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const int* d_active,
                                cudaStream_t st) {
-    z_forward64_kernel<<<dim3((g.NL + 31) / 32, 3, batch), 256, XY64_SMEM, st>>>(g, d_x, d_W, d_active);
+    z_forward64_kernel<<<dim3((g.NL + 31) / 32, 3, batch), 256, ZF64_SMEM, st>>>(g, d_x, d_W, d_active);
     return cudaGetLastError();
 }
 cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* d_W, const cplx* d_x, cplx* d_y,
@@ -273,7 +278,7 @@ cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* 
 }
 cudaError_t apply64_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(xy_conv64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZF64_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZI64_SMEM);
     return e;
 }
