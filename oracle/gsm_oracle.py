@@ -391,3 +391,85 @@ def retrieve_eps(eta, k0):
     """n_eff = eta / k0, eps_eff = n_eff^2 (PAPER.md:54, :64)."""
     n = eta / k0
     return n, n * n
+
+
+# --------------------------------------------------------------------------------------------------
+# H-field formulation, Eq. 5 (PAPER.md:56-58, :99)                         SURVEY 8(f) "next" item 1
+# --------------------------------------------------------------------------------------------------
+# H_m = H^inc_m + k_m x [ sum_m' D_{m-m'} (k_m' x H_m') ] / (k_b^2 - k_m.k_m),  D_d = delta_d0 - (eps_b/eps)_d.
+# (The Levi-Civita sums of Eq. 5 are the two cross products.)  The coefficients of the INVERSE permittivity are
+# "found analytically just in the same way" (PAPER.md:99): for inclusions eps_i in a background eps_bg,
+#   1 - eps_b/eps(r) = (1 - eps_b/eps_bg) + sum_i (eps_b/eps_bg - eps_b/eps_i) chi_i(r)
+# (exact for non-overlapping inclusions; overlapping ones superpose their terms, as in coeffs_analytic).
+def coeffs_inverse_analytic(periods, orders, shapes, eps_bg=1.0, eps_b=None) -> np.ndarray:
+    """D_d = Fourier coefficients of 1 - eps_b/eps(r), same layout as coeffs_analytic."""
+    eps_b = eps_bg if eps_b is None else eps_b
+    unit = [dict(s, eps=1.0) for s in shapes]
+    N1, N2, N3 = orders
+    D = np.zeros((2 * N1 - 1, 2 * N2 - 1, 2 * N3 - 1), dtype=np.complex128)
+    D[N1 - 1, N2 - 1, N3 - 1] = 1.0 - eps_b / eps_bg
+    for s, s1 in zip(shapes, unit):
+        # f S(d) exp(-i G.r_c) of this shape alone = coeffs_analytic with unit contrast (eps = 1, bg = 0, eps_b = 1)
+        form = coeffs_analytic(periods, orders, [s1], eps_bg=0.0, eps_b=1.0)
+        form[N1 - 1, N2 - 1, N3 - 1] += 1.0      # remove that call's background term (0 - 1)/1 at d = 0
+        D += (eps_b / eps_bg - eps_b / s["eps"]) * form
+    return D
+
+
+def coeffs_inverse_voxel(eps_grid: np.ndarray, orders, eps_b=1.0) -> np.ndarray:
+    """Direct DFT of 1 - eps_b/eps_j (same three axis sums as coeffs_voxel)."""
+    g = 1.0 - eps_b / np.asarray(eps_grid, dtype=np.complex128)
+    # coeffs_voxel forms (grid - eps_b)/eps_b; feed it a grid whose image under that map is g
+    return coeffs_voxel(eps_b * (g + 1.0), orders, eps_b)
+
+
+def cross_k(k: np.ndarray, F: np.ndarray) -> np.ndarray:
+    """(k_m x F_m) for every harmonic; k real [3, N1, N2, N3], F complex [3, N1, N2, N3]."""
+    return np.stack([k[1] * F[2] - k[2] * F[1], k[2] * F[0] - k[0] * F[2], k[0] * F[1] - k[1] * F[0]])
+
+
+def apply_operator_H(D, x, periods, k_inc, k0, eps_b, matvec=toeplitz_matvec) -> np.ndarray:
+    """y = x - k x T_D(k x x) / (k_b^2 - k.k): Eq. 5 with the unknown moved to one side."""
+    k = wavevectors(periods, x.shape[1:], k_inc)
+    kb2 = k0 * k0 * eps_b
+    den = kb2 - (k[0] ** 2 + k[1] ** 2 + k[2] ** 2)
+    return x - cross_k(k, matvec(D, cross_k(k, x))) / den[None]
+
+
+def assemble_dense_H(D, periods, orders, k_inc, k0, eps_b) -> np.ndarray:
+    """Dense matrix of Eq. 5, same index convention as assemble_dense, built entry by entry from the Levi-Civita form:
+    A[(a,m),(v,m')] = delta - sum_{b,g,s} xi_abg k_bm / (k_b^2 - k_m^2) D_{m-m'} xi_gsv k_sm'."""
+    N1, N2, N3 = orders
+    n = N1 * N2 * N3
+    i1, i2, i3 = np.meshgrid(np.arange(N1), np.arange(N2), np.arange(N3), indexing="ij")
+    i1, i2, i3 = i1.ravel(), i2.ravel(), i3.ravel()
+    T = D[(i1[:, None] - i1[None, :]) + N1 - 1, (i2[:, None] - i2[None, :]) + N2 - 1, (i3[:, None] - i3[None, :]) + N3 - 1]
+    k = wavevectors(periods, orders, k_inc).reshape(3, n)
+    den = k0 * k0 * eps_b - (k**2).sum(axis=0)
+    xi = np.zeros((3, 3, 3))
+    xi[0, 1, 2] = xi[1, 2, 0] = xi[2, 0, 1] = 1.0
+    xi[0, 2, 1] = xi[2, 1, 0] = xi[1, 0, 2] = -1.0
+    A = np.eye(3 * n, dtype=np.complex128)
+    for a in range(3):
+        for v in range(3):
+            blk = np.zeros((n, n), dtype=np.complex128)
+            for b in range(3):
+                for g_ in range(3):
+                    if xi[a, b, g_] == 0.0:
+                        continue
+                    for s in range(3):
+                        if xi[g_, s, v] == 0.0:
+                            continue
+                        blk += xi[a, b, g_] * xi[g_, s, v] * (k[b] / den)[:, None] * T * k[s][None, :]
+            A[a * n : (a + 1) * n, v * n : (v + 1) * n] -= blk
+    return A
+
+
+def solve_dense_H(D, periods, orders, k_inc, k0, eps_b, pol) -> np.ndarray:
+    A = assemble_dense_H(D, periods, orders, k_inc, k0, eps_b)
+    return np.linalg.solve(A, incident(orders, pol).ravel()).reshape((3,) + tuple(orders))
+
+
+def solve_gmres_H(D, periods, orders, k_inc, k0, eps_b, pol, tol=1e-13, max_iters=200, matvec=None):
+    mv = matvec or toeplitz_matvec
+    return gmres(lambda v: apply_operator_H(D, v, periods, k_inc, k0, eps_b, mv), incident(orders, pol), tol, max_iters)
