@@ -47,6 +47,15 @@ typedef enum {
 
 enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2 };
 
+/* Formulation solved by the plan.
+ *   GSM_FORM_E: Eq. 4, unknown E, coefficients c_d = ((eps - eps_b)/eps_b)_d            (the default)
+ *   GSM_FORM_H: Eq. 5, unknown H:
+ *       H_m - k_m x [ sum_m' D_{m-m'} (k_m' x H_m') ] / (k_b^2 - k_m.k_m) = h delta_{m,0},
+ *       D_d = delta_{d,0} - (eps_b/eps)_d, found analytically like c_d: background 1 - eps_b/eps_bg,
+ *       each inclusion adds (eps_b/eps_bg - eps_b/eps_i) x its Fourier image (exact for non-overlapping inclusions);
+ *       voxel path: transform of 1 - eps_b/eps_j.  gsm_plan_coeffs returns D_d.  `pol` is the amplitude h of H^inc. */
+enum { GSM_FORM_E = 0, GSM_FORM_H = 1 };
+
 /* One analytic inclusion ("Fourier images of sphere and polyhedron can be combined").
  * size = (R, -, -) for a sphere, semi-axes for an ellipsoid, full edge lengths for an axis-aligned box; same
  * length unit as the periods.  The inclusion's permittivity replaces the background inside it; overlapping
@@ -74,6 +83,7 @@ typedef struct {
     int max_iters;               /* GMRES basis size (unrestarted); default 64 if <= 0                         */
     int max_batch;               /* (k, omega) points solved concurrently; default 1 if <= 0                   */
     void* cuda_stream;           /* cudaStream_t to enqueue on; NULL = the legacy default stream               */
+    int formulation;             /* GSM_FORM_E (0) or GSM_FORM_H (1)                                           */
 } gsm_plan_desc;
 
 /* Build the plan on the current CUDA device: evaluate c_d (analytic closed forms or FFT of the voxel grid),

@@ -21,7 +21,15 @@ static __device__ __forceinline__ void load_tw(cplx* dst, const cplx* __restrict
 }
 
 // ---------------------------------------------------------------------------------------------------- pass 1
+// Eq. 5 (H-form): the Toeplitz product acts on (k_m x x_m); component c of that cross product
+static __device__ __forceinline__ cplx cross_k_comp(int c, double k1, double k2, double k3, cplx x0, cplx x1, cplx x2) {
+    if (c == 0) return make_double2(k2 * x2.x - k3 * x1.x, k2 * x2.y - k3 * x1.y);
+    if (c == 1) return make_double2(k3 * x0.x - k1 * x2.x, k3 * x0.y - k1 * x2.y);
+    return make_double2(k1 * x1.x - k2 * x0.x, k1 * x1.y - k2 * x0.y);
+}
+
 __global__ void __launch_bounds__(256) z_forward_kernel(ApplyGeom g, const cplx* __restrict__ x, cplx* __restrict__ W,
+                                                        const double* __restrict__ kvec,
                                                         const int* __restrict__ active) {
     const int b = blockIdx.z, c = blockIdx.y;
     if (active && !active[b]) return;
@@ -33,9 +41,21 @@ __global__ void __launch_bounds__(256) z_forward_kernel(ApplyGeom g, const cplx*
     const int nl = min(g.L, g.NL - l0);
     load_tw(tw, g.tw[2], P3);
     const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l0 * N3;
-    for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
-        const int l = i / N3, i3 = i - l * N3;
-        S[i3 * g.Lst + l] = xs[i];
+    if (!g.hform) {
+        for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
+            const int l = i / N3, i3 = i - l * N3;
+            S[i3 * g.Lst + l] = xs[i];
+        }
+    } else {
+        const cplx* xb = x + (long)b * 3 * g.n + (long)l0 * N3;
+        for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
+            const int l = i / N3, i3 = i - l * N3;
+            const int lg = l0 + l, i1 = lg / g.N2, i2 = lg - i1 * g.N2;
+            const double k1 = kvec[3 * b + 0] + (i1 + g.mmin[0]) * g.K[0];
+            const double k2 = kvec[3 * b + 1] + (i2 + g.mmin[1]) * g.K[1];
+            const double k3 = kvec[3 * b + 2] + (i3 + g.mmin[2]) * g.K[2];
+            S[i3 * g.Lst + l] = cross_k_comp(c, k1, k2, k3, xb[i], xb[g.n + i], xb[2 * g.n + i]);
+        }
     }
     __syncthreads();
     fft_forward(g.ax[2], Lines{S, g.Lst, 1}, nl, tw, N3);
@@ -146,9 +166,15 @@ __global__ void __launch_bounds__(256) z_inverse_green_kernel(ApplyGeom g, const
         const double kk[3] = {k1, k2, k3};
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            cplx num = cmul(kb2, F[c]);
-            num.x -= kk[c] * s.x;
-            num.y -= kk[c] * s.y;
+            cplx num;
+            if (g.hform) {   // Eq. 5: y = x - k x F / (k_b^2 - k.k) = x + (k x F) / (k.k - k_b^2)
+                const cplx t = cross_k_comp(c, k1, k2, k3, F0, F1, F2);
+                num = make_double2(-t.x, -t.y);
+            } else {
+                num = cmul(kb2, F[c]);
+                num.x -= kk[c] * s.x;
+                num.y -= kk[c] * s.y;
+            }
             const cplx q = cmul(num, rden);
             const cplx xv = x[base + c * g.n + i];
             y[base + c * g.n + i] = make_double2(xv.x - q.x, xv.y - q.y);
@@ -188,8 +214,8 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
         const double* k0 = d_k0 + b0;
         const int* act = d_active ? d_active + b0 : nullptr;
         { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
-          if (g.chat64) launch_z_forward64(g, nb, x, d_W, act, st);
-          else z_forward_kernel<<<dim3(nlt, 3, nb), 256, smem_pass1(g), st>>>(g, x, d_W, act); }
+          if (g.chat64) launch_z_forward64(g, nb, x, d_W, kv, act, st);
+          else z_forward_kernel<<<dim3(nlt, 3, nb), 256, smem_pass1(g), st>>>(g, x, d_W, kv, act); }
         { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
           if (g.chat64) launch_xy_conv64(g, nb, d_W, g.chat64, act, st);
           else if (g.chat128) launch_xy_conv128(g, nb, d_W, g.chat128, act, st);

@@ -115,8 +115,10 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
 #ifndef ZF64_MINB
 #define ZF64_MINB 4
 #endif
+template <bool HFORM>
 __global__ void __launch_bounds__(256, ZF64_MINB) z_forward64_kernel(ApplyGeom g, const cplx* __restrict__ x,
-                                                                     cplx* __restrict__ W, const int* __restrict__ active) {
+                                                                     cplx* __restrict__ W, const double* __restrict__ kvec,
+                                                                     const int* __restrict__ active) {
     const int b = blockIdx.z, c = blockIdx.y;
     if (active && !active[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -130,10 +132,30 @@ __global__ void __launch_bounds__(256, ZF64_MINB) z_forward64_kernel(ApplyGeom g
     const int l0 = blockIdx.x * 32, line = warp * 4 + ln, l = l0 + line;
     const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l * N3;
     cplx a[8];
+    if (!HFORM) {
 #pragma unroll
-    for (int p = 0; p < 4; ++p) {
-        const int i3 = u + 8 * p;
-        a[p] = (l < NL && i3 < N3) ? xs[i3] : make_double2(0.0, 0.0);
+        for (int p = 0; p < 4; ++p) {
+            const int i3 = u + 8 * p;
+            a[p] = (l < NL && i3 < N3) ? xs[i3] : make_double2(0.0, 0.0);
+        }
+    } else {   // Eq. 5: the Toeplitz product acts on (k x x); component c needs the two other components of x
+        const int c1 = c == 2 ? 0 : c + 1, c2 = c1 == 2 ? 0 : c1 + 1;
+        const int i1 = l / g.N2, i2 = l - i1 * g.N2;
+        const double kk[3] = {kvec[3 * b + 0] + (i1 + g.mmin[0]) * g.K[0], kvec[3 * b + 1] + (i2 + g.mmin[1]) * g.K[1],
+                              kvec[3 * b + 2] + g.mmin[2] * g.K[2]};
+        const cplx* x1 = x + ((long)b * 3 + c1) * g.n + (long)l * N3;
+        const cplx* x2 = x + ((long)b * 3 + c2) * g.n + (long)l * N3;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const int i3 = u + 8 * p;
+            if (l < NL && i3 < N3) {
+                const double ka = c1 == 2 ? kk[2] + i3 * g.K[2] : kk[c1], kb = c2 == 2 ? kk[2] + i3 * g.K[2] : kk[c2];
+                const cplx v1 = x1[i3], v2 = x2[i3];   // (k x x)_c = k_c1 x_c2 - k_c2 x_c1
+                a[p] = make_double2(ka * v2.x - kb * v1.x, ka * v2.y - kb * v1.y);
+            } else {
+                a[p] = make_double2(0.0, 0.0);
+            }
+        }
     }
     fwd64_group(a, tw, sc, u);
     __syncthreads();   // every warp is done with its scratch lines: the tile may overwrite them
@@ -231,9 +253,15 @@ __global__ void __launch_bounds__(256, 2) z_inverse_green64_kernel(ApplyGeom g, 
         const cplx Fc[3] = {F0, F1, F2};
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            cplx num = cmul(kb2, Fc[c]);
-            num.x -= kk[c] * s.x;
-            num.y -= kk[c] * s.y;
+            cplx num;
+            if (g.hform) {   // Eq. 5: y = x + (k x F) / (k.k - k_b^2)
+                const int c1 = c == 2 ? 0 : c + 1, c2 = c1 == 2 ? 0 : c1 + 1;
+                num = make_double2(-(kk[c1] * Fc[c2].x - kk[c2] * Fc[c1].x), -(kk[c1] * Fc[c2].y - kk[c2] * Fc[c1].y));
+            } else {
+                num = cmul(kb2, Fc[c]);
+                num.x -= kk[c] * s.x;
+                num.y -= kk[c] * s.y;
+            }
             const cplx q = cmul(num, rden);
             const cplx xv = x[base + c * g.n + i3];
             y[base + c * g.n + i3] = make_double2(xv.x - q.x, xv.y - q.y);
@@ -265,9 +293,11 @@ cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cpl
 }
 static const size_t ZF64_SMEM = sizeof(cplx) * (32 * SC_LINE);   // >= 64 * 32 tile
 static const size_t ZI64_SMEM = sizeof(cplx) * (2 * 64 * 32 + 32 * SC_LINE);
-cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const int* d_active,
-                               cudaStream_t st) {
-    z_forward64_kernel<<<dim3((g.NL + 31) / 32, 3, batch), 256, ZF64_SMEM, st>>>(g, d_x, d_W, d_active);
+cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const double* d_kvec,
+                               const int* d_active, cudaStream_t st) {
+    const dim3 grid((g.NL + 31) / 32, 3, batch);
+    if (g.hform) z_forward64_kernel<true><<<grid, 256, ZF64_SMEM, st>>>(g, d_x, d_W, d_kvec, d_active);
+    else z_forward64_kernel<false><<<grid, 256, ZF64_SMEM, st>>>(g, d_x, d_W, d_kvec, d_active);
     return cudaGetLastError();
 }
 cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* d_W, const cplx* d_x, cplx* d_y,
@@ -278,7 +308,8 @@ cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* 
 }
 cudaError_t apply64_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(xy_conv64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XY64_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZF64_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZF64_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(z_forward64_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZF64_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZI64_SMEM);
     return e;
 }

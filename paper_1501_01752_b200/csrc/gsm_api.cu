@@ -144,7 +144,12 @@ static gsm_status build_coeffs(gsm_plan* plan) {
             ShapeDev& q = hs[i];
             q.kind = s.kind;
             for (int a = 0; a < 3; ++a) { q.c[a] = s.center[a]; q.s[a] = s.size[a]; }
-            const cplx del = cdivh(s.eps_re - d.eps_bg_re, s.eps_im - d.eps_bg_im, d.eps_b_re, d.eps_b_im);
+            cplx del = cdivh(s.eps_re - d.eps_bg_re, s.eps_im - d.eps_bg_im, d.eps_b_re, d.eps_b_im);
+            if (d.formulation == GSM_FORM_H) {   // eps_b/eps_bg - eps_b/eps_i
+                const cplx a = cdivh(d.eps_b_re, d.eps_b_im, d.eps_bg_re, d.eps_bg_im);
+                const cplx b = cdivh(d.eps_b_re, d.eps_b_im, s.eps_re, s.eps_im);
+                del = make_double2(a.x - b.x, a.y - b.y);
+            }
             q.dre = del.x; q.dim = del.y;
             if (s.kind == GSM_SPHERE) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[0] * s.size[0] / vol;
             else if (s.kind == GSM_ELLIPSOID) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[1] * s.size[2] / vol;
@@ -154,7 +159,9 @@ static gsm_status build_coeffs(gsm_plan* plan) {
         ShapeDev* dsh = nullptr;
         CK(cudaMalloc(&dsh, sizeof(ShapeDev) * hs.size()));
         cudaError_t e = cudaMemcpyAsync(dsh, hs.data(), sizeof(ShapeDev) * hs.size(), cudaMemcpyHostToDevice, plan->stream);
-        const cplx c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_b_re, d.eps_b_im);
+        cplx c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_b_re, d.eps_b_im);
+        if (d.formulation == GSM_FORM_H)     // 1 - eps_b/eps_bg = (eps_bg - eps_b)/eps_bg
+            c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_bg_re, d.eps_bg_im);
         if (e == cudaSuccess) {
             ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
             e = launch_coeffs_analytic(dsh, d.n_shapes, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
@@ -187,7 +194,7 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     cplx* grid = plan->vgrid;
     cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
     ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
-    if (e == cudaSuccess) e = launch_voxel_prepare(grid, (long)nv, d.eps_b_re, d.eps_b_im, plan->stream);
+    if (e == cudaSuccess) e = launch_voxel_prepare(grid, (long)nv, d.eps_b_re, d.eps_b_im, d.formulation == GSM_FORM_H, plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0] * V[1], vax[2], 1, vtw[2], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, (long)V[0], vax[1], V[2], vtw[1], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(grid, 1, vax[0], (long)V[1] * V[2], vtw[0], plan->stream);
@@ -265,6 +272,9 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
             CK(upload_twiddles(plan, g.ax[a].P, &g.tw[a]));
         }
         g.epsb_re = desc->eps_b_re; g.epsb_im = desc->eps_b_im;
+        if (desc->formulation != GSM_FORM_E && desc->formulation != GSM_FORM_H)
+            return fail(plan, GSM_E_INVALID, "formulation must be GSM_FORM_E or GSM_FORM_H");
+        g.hform = desc->formulation == GSM_FORM_H;
         g.L = std::min(g.NL, g.ax[2].P >= 128 ? 16 : 32);
         g.Lst = odd_at_least(g.L);
         g.RS3 = odd_at_least(3 * g.L);

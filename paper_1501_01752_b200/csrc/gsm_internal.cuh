@@ -44,6 +44,7 @@ struct ApplyGeom {
     int N1, N2, N3;      // harmonics kept
     int NL;              // N1*N2 = number of z-lines per component
     long n;              // N1*N2*N3
+    int hform;           // 0: Eq. 4 (E, Green dyadic); 1: Eq. 5 (H, cross products around the Toeplitz product)
     int sub;             // solves per pass through the workspace W (L2-resident sub-batches)
     int L;               // z-lines per CTA in passes 1 and 3
     int Lst;             // odd row stride (>= L) of the pass-1 tile
@@ -86,8 +87,8 @@ cudaError_t launch_xy_conv128(const ApplyGeom& g, int batch, cplx* d_W, const cp
 bool apply64_usable(const ApplyGeom& g);
 cudaError_t apply64_init_attributes();
 cudaError_t launch_chat64_layout(const cplx* d_chat, cplx* d_chat64, cudaStream_t st);
-cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const int* d_active,
-                               cudaStream_t st);
+cudaError_t launch_z_forward64(const ApplyGeom& g, int batch, const cplx* d_x, cplx* d_W, const double* d_kvec,
+                               const int* d_active, cudaStream_t st);
 cudaError_t launch_z_inverse_green64(const ApplyGeom& g, int batch, const cplx* d_W, const cplx* d_x, cplx* d_y,
                                      const double* d_kvec, const double* d_k0, const int* d_active, cudaStream_t st);
 cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat64, const int* d_active,
@@ -106,7 +107,7 @@ cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, double
 cudaError_t launch_fft_axis(cplx* d_data, long outer, const AxisPlan& ax, long inner, const cplx* d_tw, cudaStream_t st);
 cudaError_t launch_embed(const cplx* d_coef, const int N[3], const int P[3], cplx* d_pad, cudaStream_t st);
 cudaError_t launch_chat_layout(const cplx* d_padfft, const int P[3], cplx* d_chat, cudaStream_t st);
-cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, cudaStream_t st);
+cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, int hform, cudaStream_t st);
 cudaError_t launch_voxel_extract(const cplx* d_gridfft, const int Nv[3], const int N[3], const int* d_pos1,
                                  const int* d_pos2, const int* d_pos3, cplx* d_coef, cudaStream_t st);
 

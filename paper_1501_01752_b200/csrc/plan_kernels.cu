@@ -126,17 +126,22 @@ cudaError_t launch_chat_layout(const cplx* d_padfft, const int P[3], cplx* d_cha
     return cudaGetLastError();
 }
 
-// voxel path: g_j = (eps_j - eps_b) / eps_b in place
-__global__ void voxel_prepare_kernel(cplx* __restrict__ grid, long count, double br, double bi) {
+// voxel path: g_j = (eps_j - eps_b) / eps_b (Eq. 4) or 1 - eps_b / eps_j (Eq. 5) in place
+__global__ void voxel_prepare_kernel(cplx* __restrict__ grid, long count, double br, double bi, int hform) {
     const double inv = 1.0 / (br * br + bi * bi);
     for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < count; i += (long)gridDim.x * blockDim.x) {
         const cplx e = grid[i];
+        if (hform) {   // 1 - eps_b / eps = (eps - eps_b) / eps
+            const double nr = e.x - br, ni = e.y - bi, ie = 1.0 / (e.x * e.x + e.y * e.y);
+            grid[i] = make_double2((nr * e.x + ni * e.y) * ie, (ni * e.x - nr * e.y) * ie);
+            continue;
+        }
         const double nr = e.x - br, ni = e.y - bi;
         grid[i] = make_double2((nr * br + ni * bi) * inv, (ni * br - nr * bi) * inv);
     }
 }
-cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, cudaStream_t st) {
-    voxel_prepare_kernel<<<1024, 256, 0, st>>>(d_grid, count, epsb_re, epsb_im);
+cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, int hform, cudaStream_t st) {
+    voxel_prepare_kernel<<<1024, 256, 0, st>>>(d_grid, count, epsb_re, epsb_im, hform);
     return cudaGetLastError();
 }
 

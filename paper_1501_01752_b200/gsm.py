@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgsm_b200.so")
 
 OK, NOT_CONVERGED, E_INVALID, E_ALLOC, E_CUDA, E_SINGULAR_BASIS = 0, 1, -1, -2, -3, -4
 SPHERE, ELLIPSOID, BOX = 0, 1, 2
+FORM_E, FORM_H = 0, 1
 
 
 class GsmError(RuntimeError):
@@ -36,7 +37,8 @@ class _PlanDesc(C.Structure):
                 ("eps_b_re", C.c_double), ("eps_b_im", C.c_double),
                 ("n_shapes", C.c_int), ("shapes", C.POINTER(_Shape)),
                 ("voxels", C.c_int * 3), ("eps_grid_host", C.c_void_p),
-                ("max_iters", C.c_int), ("max_batch", C.c_int), ("cuda_stream", C.c_void_p)]
+                ("max_iters", C.c_int), ("max_batch", C.c_int), ("cuda_stream", C.c_void_p),
+                ("formulation", C.c_int)]
 
 
 def _load():
@@ -91,12 +93,13 @@ class Plan:
     """gsm_plan: one periodic cell (periods, orders, shapes or voxel grid) on the current CUDA device."""
 
     def __init__(self, periods, orders, shapes=None, eps_bg=1.0, eps_b=None, voxels=None, max_iters=64, max_batch=1,
-                 stream=None):
+                 stream=None, formulation=FORM_E):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1501_01752_b200.gsm needs a CUDA device; there is no CPU fallback")
         self._torch = torch
         self.stream = stream
+        self.formulation = int(formulation)
         self.orders = tuple(int(n) for n in orders)
         d, keep = self._desc(periods, shapes, eps_bg, eps_b, voxels, max_iters, max_batch)
         self.n = int(np.prod(self.orders))
@@ -142,6 +145,7 @@ class Plan:
             keep = arr
         d.max_iters, d.max_batch = int(max_iters), int(max_batch)
         d.cuda_stream = self.stream.cuda_stream if self.stream is not None else None
+        d.formulation = self.formulation
         return d, keep
 
     def set_cell(self, periods, shapes=None, eps_bg=1.0, eps_b=None, voxels=None):
@@ -248,7 +252,7 @@ def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):
     return eta, zeta, best.value
 
 
-def plan_from_geometry(geo, max_iters=64, max_batch=1, stream=None) -> Plan:
+def plan_from_geometry(geo, max_iters=64, max_batch=1, stream=None, formulation=FORM_E) -> Plan:
     """Plan for a workloads.Geometry (seeded input description; holds no arithmetic of the method)."""
     return Plan(geo.periods, geo.orders, shapes=geo.shapes, eps_bg=geo.eps_bg, eps_b=geo.eps_b, voxels=geo.voxels,
-                max_iters=max_iters, max_batch=max_batch, stream=stream)
+                max_iters=max_iters, max_batch=max_batch, stream=stream, formulation=formulation)
