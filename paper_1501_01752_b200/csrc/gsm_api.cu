@@ -24,6 +24,7 @@ struct gsm_plan {
     std::vector<void*> allocs;    // every device allocation, freed in destroy
     long long device_bytes = 0;
     Profiler prof;
+    cudaEvent_t iter_ev[2] = {nullptr, nullptr};   // completion of the per-iteration nactive read-back
     cplx* chat64 = nullptr;
     cplx* chat128 = nullptr;
     int* gen128[2] = {nullptr, nullptr};
@@ -333,6 +334,8 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &plan->d_resid, (size_t)B));
         plan->pinned_bytes = sizeof(double) * ((size_t)B * (12 + kd.mmax) + 16);
         CK(cudaMallocHost(&plan->pinned, plan->pinned_bytes));
+        CK(cudaEventCreateWithFlags(&plan->iter_ev[0], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&plan->iter_ev[1], cudaEventDisableTiming));
         return GSM_OK;
     };
     st = body();
@@ -349,6 +352,7 @@ extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
     if (!plan) return GSM_E_INVALID;
     cudaStreamSynchronize(plan->stream);
     plan->prof.destroy();
+    for (cudaEvent_t e : plan->iter_ev) if (e) cudaEventDestroy(e);
     for (void* p : plan->allocs) cudaFree(p);
     if (plan->pinned) cudaFreeHost(plan->pinned);
     delete plan;
@@ -454,10 +458,16 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
             CK(launch_givens(kd, ks, nb, j, st, prof));
             CK(launch_normalize(kd, ks, nb, j, st, prof, nact));
         }
-        CK(cudaMemcpyAsync(pin_i, ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-        nact = pin_i[0];
-        if (nact <= 0) break;
+        // The count of solves still iterating comes back one iteration late: iteration j + 1 is enqueued before the
+        // host looks at the count after iteration j - 1, so launches never wait for a round trip.  If everything had
+        // already converged, the extra iteration's CTAs find their `active` flags cleared and exit at once.
+        CK(cudaMemcpyAsync(pin_i + (j & 1), ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(plan->iter_ev[j & 1], st));
+        if (j >= 1) {
+            CK(cudaEventSynchronize(plan->iter_ev[(j - 1) & 1]));
+            nact = pin_i[(j - 1) & 1];
+            if (nact <= 0) break;
+        }
     }
     CK(launch_backsolve(kd, ks, nb, st, prof));
     CK(launch_combine(kd, ks, nb, d_E, st, prof));
