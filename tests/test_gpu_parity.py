@@ -170,3 +170,46 @@ def test_apply_rejects_singular_basis_and_bad_batch():
         plan.apply(np.zeros((3, 3)), np.ones(3), x3)
     assert e.value.status == gsm.E_INVALID
     plan.close()
+
+
+def test_set_cell_rebuilds_harmonics_in_place():
+    """gsm_plan_set_cell re-runs step a0 for a new cell (analytic -> analytic -> voxel) without touching the workspaces."""
+    g1 = wl.sphere_lattice((7, 7, 7))
+    plan = gsm.plan_from_geometry(g1, max_batch=2)
+    bytes0 = plan.info()["device_bytes"]
+    g2 = wl.Geometry("other", (0.25, 0.2, 0.3), (7, 7, 7), wl.ellipsoid_lattice().shapes, 1.2, 1.1, None, ())
+    plan.set_cell(g2.periods, shapes=g2.shapes, eps_bg=g2.eps_bg, eps_b=g2.eps_b)
+    assert np.max(np.abs(plan.coeffs() - oracle_coeffs(g2))) <= 1e-14
+    x = wl.random_field(1, g2.orders, 8)
+    kb, k0 = np.array([[0.2, 0.1, 1.2 * TWO_PI]]), np.array([TWO_PI])
+    y = plan.apply(kb, k0, torch.from_numpy(x).cuda()).cpu().numpy()[0]
+    assert rel(y, orc.apply_operator(oracle_coeffs(g2), x[0], g2.periods, kb[0], k0[0], g2.eps_b)) <= 1e-12
+    rng = np.random.default_rng(3)
+    grid = (1.0 + 5.0 * rng.random((16, 16, 16))).astype(np.complex128)
+    g3 = wl.Geometry("vox", (0.2, 0.2, 0.2), (7, 7, 7), [], 1.0, 1.0, grid, ())
+    plan.set_cell(g3.periods, eps_bg=1.0, eps_b=1.0, voxels=grid)
+    assert np.max(np.abs(plan.coeffs() - oracle_coeffs(g3))) <= 1e-13 * np.max(np.abs(oracle_coeffs(g3)))
+    y = plan.apply(kb, k0, torch.from_numpy(x).cuda()).cpu().numpy()[0]
+    assert rel(y, orc.apply_operator(oracle_coeffs(g3), x[0], g3.periods, kb[0], k0[0], g3.eps_b)) <= 1e-12
+    assert plan.info()["device_bytes"] - bytes0 <= 16 * (16 ** 3 + 3 * 16) + 3 * 4 * 16 + 64   # only the voxel staging was added
+    assert gsm._lib.gsm_plan_set_cell(plan._h, None) == gsm.E_INVALID
+    plan.close()
+
+
+def test_launch_accounting_and_event_profile():
+    """Every kernel of a solve is counted per class; with profiling on, each class reports device time and bytes."""
+    geo = wl.sphere_lattice((7, 7, 7))
+    plan = gsm.plan_from_geometry(geo, max_batch=1)
+    plan.profile_read(reset=True)
+    plan.profile(True)
+    E, hist, iters, resid, st = plan.solve([0, 0, 1.2 * TWO_PI], TWO_PI, [1.0, 0, 0], tol=1e-10)
+    pr = plan.profile_read(reset=True)
+    plan.profile(False)
+    napply = pr["z_forward"][0]
+    assert napply == pr["xy_conv"][0] == pr["z_inverse_green"][0]
+    assert iters + 1 <= napply <= iters + 2          # one apply per iteration (+ at most one overlapped extra) + the residual check
+    steps = pr["arnoldi_mgs"][0] if pr["arnoldi_mgs"][0] else pr["sweep_dots"][0]
+    assert iters <= steps <= iters + 1
+    assert all(ms > 0 for (n, ms, by) in pr.values() if n > 0)
+    assert pr["xy_conv"][2] > 0 and plan.info()["launches"] == 0       # bytes were accounted; the reset cleared the counters
+    plan.close()
