@@ -257,3 +257,78 @@ def test_degenerate_inputs_empty_scan_zero_source_and_largest_orders():
     with pytest.raises(gsm.GsmError) as e:
         gsm.Plan((0.2, 0.2, 0.2), (65, 1, 1), shapes=geo.shapes)
     assert e.value.status == gsm.E_INVALID
+
+
+def test_config2_laminate_in_plane_te_tm_vs_dense_lu():
+    """BASELINE config 2, propagation along x (in the layer planes): a = y (TE) and a = z (TM), fields vs dense LU."""
+    geo = wl.laminate((1, 1, 63))
+    plan = gsm.plan_from_geometry(geo, max_iters=120, max_batch=6)
+    c = coeffs(geo)
+    k0 = TWO_PI * 0.25 * 24 / 64
+    kb = np.zeros((6, 3)); pol = np.zeros((6, 3), dtype=complex)
+    ns = [1.9, 2.1, 2.3, 1.2, 1.3, 1.45]                  # TE points around n ~ sqrt(5), TM points around n ~ sqrt(1.8)
+    for i, n in enumerate(ns):
+        kb[i, 0] = n * k0
+        pol[i, 1 if i < 3 else 2] = 1.0
+    fields = torch.empty((6, 3, 1, 1, 63), dtype=torch.complex128, device="cuda")
+    resp, iters, resid, st = plan.scan(kb, np.full(6, k0), pol, tol=1e-12, fields=fields)
+    assert st == gsm.OK and np.all(resid <= 1e-10)
+    F = fields.cpu().numpy()
+    for i in range(6):
+        ref = orc.solve_dense(c, geo.periods, geo.orders, kb[i], k0, geo.eps_b, pol[i])
+        assert rel(F[i], ref) <= 1e-9
+    plan.close()
+
+
+def test_config4_woodpile_31cubed_three_directions():
+    """BASELINE config 4: one (k, omega) point per search direction (z,x), (x,y), (x,z) in one batch.  The (z,x) solve is
+    compared with the oracle's GMRES; all three are checked against the equation itself at sampled harmonics with the
+    oracle's O(n) row sums (A E = b)."""
+    geo = wl.woodpile((31, 31, 31))
+    plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=3)
+    c = coeffs(geo)
+    pts = [(2, 0, 1.35), (0, 1, 1.36), (0, 2, 1.27)]
+    kb = np.zeros((3, 3)); pol = np.zeros((3, 3), dtype=complex)
+    for i, (pa, qa, ni) in enumerate(pts):
+        kb[i, pa] = ni * TWO_PI
+        pol[i, qa] = 1.0
+    fields = torch.empty((3, 3, 31, 31, 31), dtype=torch.complex128, device="cuda")
+    resp, iters, resid, st = plan.scan(kb, np.full(3, TWO_PI), pol, tol=1e-12, fields=fields)
+    assert st == gsm.OK and np.all(resid <= 1e-10)
+    F = fields.cpu().numpy()
+    ref, _, oit = orc.solve_gmres(c, geo.periods, geo.orders, kb[0], TWO_PI, geo.eps_b, pol[0], tol=1e-13, max_iters=150,
+                                  matvec=orc.toeplitz_matvec_c)
+    assert rel(F[0], ref) <= 1e-9 and abs(int(iters[0]) - oit) <= 5
+    _check_equation_rows(geo, c, F, kb, np.full(3, TWO_PI), pol, 10)
+    plan.close()
+
+
+def _check_equation_rows(geo, c, F, kb, k0, pol, nsamp):
+    """(A E)_m = b_m at sampled harmonics, A E evaluated by the oracle's row sum (no FFT, O(n) per row)."""
+    rng = np.random.default_rng(17)
+    N = geo.orders
+    i0 = tuple((n - 1) // 2 for n in N)
+    for b in range(F.shape[0]):
+        k = orc.wavevectors(geo.periods, N, kb[b])
+        kb2 = k0[b] ** 2 * geo.eps_b
+        scale = np.abs(F[b]).max()
+        for s in [i0, (0, 0, 0)] + [tuple(int(rng.integers(0, N[a])) for a in range(3)) for _ in range(nsamp)]:
+            T = orc.toeplitz_row(c, F[b], s)
+            km = k[(slice(None),) + s]
+            lhs = F[b][(slice(None),) + s] - (kb2 * T - km * np.dot(km, T)) / (np.dot(km, km) - kb2)
+            rhs = pol[b] if s == i0 else np.zeros(3)
+            assert np.max(np.abs(lhs - rhs)) <= 1e-9 * max(1.0, scale)
+
+
+def test_config5b_63cubed_single_solve_satisfies_the_equation():
+    """BASELINE config 5b: one solve at 63^3 orders (128-point xy fast path, generic z passes, two-sweep Gram-Schmidt).
+    The oracle cannot afford a solve at this size; the returned field is checked against the equation at sampled
+    harmonics through the oracle's row sums, and against the solver's own true residual."""
+    geo = wl.voxel_composite((63, 63, 63), nv=128)
+    plan = gsm.plan_from_geometry(geo, max_iters=80, max_batch=1)
+    kb = np.array([0.0, 0.0, 1.12 * TWO_PI]); pol = np.array([1.0, 0, 0], dtype=complex)
+    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    assert st == gsm.OK and resid <= 1e-10 and 20 <= iters <= 70 and np.all(np.diff(hist) <= 1e-15)
+    c = coeffs(geo)
+    _check_equation_rows(geo, c, E.cpu().numpy()[None], kb[None], np.array([TWO_PI]), pol[None], 8)
+    plan.close()
