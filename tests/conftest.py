@@ -8,6 +8,14 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+# Build steps run before any test module is imported (the binding refuses to import without its library; the built
+# .so is git-ignored): nvcc -> libgsm_b200.so, gcc -> the oracle's C helper.  Both are no-ops when up to date.
+from paper_1501_01752_b200.build import build_cuda, build_oracle  # noqa: E402
+
+build_cuda()
+build_oracle()
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200)")
 
