@@ -114,7 +114,7 @@ cudaError_t launch_voxel_extract(const cplx* d_gridfft, const int Nv[3], const i
 // ---- launches implemented in krylov.cu -------------------------------------------------------------------------
 struct KrylovState {   // all device pointers, one entry (or row) per solve of the batch
     cplx* basis;       // [ld][batch][vlen]
-    cplx* part;        // [batch][nchunk][2*ld] partial inner products of sweep 1 / partial norms of sweep 2
+    cplx* part;        // [batch][2*ld][nchunk] partial inner products of sweep 1 / partial norms of sweep 2 (row 0)
     cplx* gram;        // [batch][ld][ld]   gram[j][i] = <v_i, v_j>, i <= j
     cplx* hcol;        // [batch][ld]       current Hessenberg column after Gram-Schmidt
     cplx* R;           // [batch][ld][mmax] rotated Hessenberg (upper triangular)

@@ -85,15 +85,15 @@ __global__ void __launch_bounds__(KT) sweep_dots_kernel(KrylovDims d, KrylovStat
         }
     }
     __syncthreads();
-    cplx* out = s.part + ((long)b * d.nchunk + blockIdx.x) * 2 * d.ld;
+    cplx* out = s.part + (long)b * 2 * d.ld * d.nchunk + blockIdx.x;   // part[b][q][chunk]: reductions read contiguously
     for (int i = threadIdx.x; i <= j; i += KT) {
         double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
         for (int wq = 0; wq < KT / 32; ++wq) {
             const double* r = red + ((long)wq * (j + 1) + i) * 4;
             a0 += r[0]; a1 += r[1]; g0 += r[2]; g1 += r[3];
         }
-        out[2 * i] = make_double2(a0, a1);
-        out[2 * i + 1] = make_double2(g0, g1);
+        out[(long)(2 * i) * d.nchunk] = make_double2(a0, a1);
+        out[(long)(2 * i + 1) * d.nchunk] = make_double2(g0, g1);
     }
 }
 
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(KT) sweep_dots_kernel(KrylovDims d, KrylovStat
 // HS_T threads: warp w reduces the partials of entries i = w, w + HS_T/32, ... (lanes stride over the chunks, fixed
 // shuffle tree: deterministic), then warp 0 runs the recurrence.
 #define HS_T 256
-__global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j) {
+__global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j, int stage) {
     const int b = blockIdx.x;
     if (!s.active[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -110,9 +110,9 @@ __global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int i = warp; i <= j; i += HS_T / 32) {
         double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
-        const cplx* p = s.part + (long)b * d.nchunk * 2 * d.ld + 2 * i;
+        const cplx* p = s.part + ((long)b * 2 * d.ld + 2 * i) * d.nchunk;
         for (int c = lane; c < d.nchunk; c += 32) {
-            const cplx a = p[(long)c * 2 * d.ld], g = p[(long)c * 2 * d.ld + 1];
+            const cplx a = p[c], g = p[d.nchunk + c];
             a0 += a.x; a1 += a.y; g0 += g.x; g1 += g.y;
         }
         a0 = warp_sum(a0); a1 = warp_sum(a1); g0 = warp_sum(g0); g1 = warp_sum(g1);
@@ -121,14 +121,26 @@ __global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState 
             gT[(long)i * d.ld + j] = make_double2(g0, g1);
         }
     }
+    // stage the Gram rows the recurrence needs (k < i <= j) in shared memory: the recurrence is a chain of j dependent
+    // steps, and a global-memory load per step would cost an L2 round trip each
+    const cplx* gs = gT;                             // stage == 0: basis too long for shared memory, read the rows from global
+    if (stage) {
+        cplx* gw = dd + d.ld;                        // [j][ld] rows 0..j-1
+        for (int q = threadIdx.x; q < j * (j + 1); q += HS_T) {
+            const int k = q / (j + 1), i = q - k * (j + 1);
+            if (i > k && i < j) gw[k * d.ld + i] = gT[(long)k * d.ld + i];
+        }
+        __syncthreads();                             // also orders the column-j entries written above
+        for (int q = threadIdx.x; q < j; q += HS_T) gw[q * d.ld + j] = gT[(long)q * d.ld + j];
+        gs = gw;
+    }
     __syncthreads();
     if (warp != 0) return;
     // column-oriented recurrence: once h_k is final, every later d_i loses h_k <v_i, v_k> = h_k conj(<v_k, v_i>)
     for (int k = 0; k < j; ++k) {
         const cplx hk = dd[k];
         for (int i = k + 1 + lane; i <= j; i += 32) {
-            const cplx gki = gT[(long)k * d.ld + i];
-            const cplx t = cmulc(hk, gki);
+            const cplx t = cmulc(hk, gs[(long)k * d.ld + i]);
             dd[i] = make_double2(dd[i].x - t.x, dd[i].y - t.y);
         }
         __syncwarp();
@@ -182,7 +194,7 @@ __global__ void __launch_bounds__(KT) sweep_update_kernel(KrylovDims d, KrylovSt
     if (threadIdx.x == 0) {
         double t = 0.0;
         for (int q = 0; q < KT / 32; ++q) t += wsum[q];
-        s.part[((long)b * d.nchunk + blockIdx.x) * 2 * d.ld] = make_double2(t, 0.0);
+        s.part[(long)b * 2 * d.ld * d.nchunk + blockIdx.x] = make_double2(t, 0.0);
     }
 }
 
@@ -191,7 +203,7 @@ __global__ void givens_kernel(KrylovDims d, KrylovState s, int batch, int j) {  
     const int b = blockIdx.x;
     if (!s.active[b]) return;
     double nn = 0.0;
-    for (int c = threadIdx.x; c < d.nchunk; c += 32) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    for (int c = threadIdx.x; c < d.nchunk; c += 32) nn += s.part[(long)b * 2 * d.ld * d.nchunk + c].x;
     nn = warp_sum(nn);
     if (threadIdx.x != 0) return;
     givens_step(d, s, b, j, s.hcol + (long)b * d.ld, sqrt(nn), s.cs + (long)b * d.mmax, s.sn + (long)b * d.mmax);
@@ -287,14 +299,14 @@ __global__ void __launch_bounds__(KT) resid_part_kernel(KrylovDims d, KrylovStat
     if (threadIdx.x == 0) {
         double t = 0.0;
         for (int q = 0; q < KT / 32; ++q) t += wsum[q];
-        s.part[((long)b * d.nchunk + blockIdx.x) * 2 * d.ld] = make_double2(t, 0.0);
+        s.part[(long)b * 2 * d.ld * d.nchunk + blockIdx.x] = make_double2(t, 0.0);
     }
 }
 __global__ void resid_final_kernel(KrylovDims d, KrylovState s, int batch, double* __restrict__ resid) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
     double nn = 0.0;
-    for (int c = 0; c < d.nchunk; ++c) nn += s.part[((long)b * d.nchunk + c) * 2 * d.ld].x;
+    for (int c = 0; c < d.nchunk; ++c) nn += s.part[(long)b * 2 * d.ld * d.nchunk + c].x;
     resid[b] = s.beta[b] > 0.0 ? sqrt(nn) / s.beta[b] : 0.0;
 }
 
@@ -303,6 +315,7 @@ __global__ void resid_final_kernel(KrylovDims d, KrylovState s, int batch, doubl
 
 cudaError_t krylov_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(sweep_dots_kernel<GSM_E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     return e;
 }
 cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st, Profiler* prof) {
@@ -318,7 +331,10 @@ cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int bat
 }
 cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
     ProfScope ps_(prof, KC_HSOLVE, st);
-    hsolve_kernel<<<batch, HS_T, sizeof(cplx) * d.ld, st>>>(d, s, batch, j);
+    size_t smem = sizeof(cplx) * d.ld * (size_t)(j + 1);
+    const int stage = smem <= 200 * 1024;
+    if (!stage) smem = sizeof(cplx) * d.ld;
+    hsolve_kernel<<<batch, HS_T, smem, st>>>(d, s, batch, j, stage);
     return cudaGetLastError();
 }
 cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
