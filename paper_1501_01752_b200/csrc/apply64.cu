@@ -59,11 +59,7 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
     }
     __syncthreads();
     // ---- x: forward, multiply by the coefficient spectrum, inverse
-#ifdef XY64_UNROLL
-#pragma unroll
-#else
 #pragma unroll 1
-#endif
     for (int round = 0; round < 2; ++round) {
         const int r = (round * 8 + warp) * 4 + ln;
         cplx* Ar = A + r * 32;
@@ -74,18 +70,9 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
             a[p] = (i1 < N1) ? Ar[(i1 + rot) & 31] : make_double2(0.0, 0.0);
         }
         const cplx* cp = chat64 + ((long)(pos3 * 64 + r) * 64) + u;
-#ifdef XY64_PREFETCH
-        cplx ch[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) ch[q] = __ldg(cp + 8 * q);
-        fwd64_group(a, tw, sc, u);
-#pragma unroll
-        for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], ch[q]);
-#else
         fwd64_group(a, tw, sc, u);
 #pragma unroll
         for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], __ldg(cp + 8 * q));
-#endif
         inv64_group(a, tw, sc, u);
 #pragma unroll
         for (int p = 0; p < 4; ++p) {

@@ -617,7 +617,6 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
     if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(plan, GSM_E_INVALID, "eps_b must be non-zero");
     if (desc->eps_grid_host == nullptr && (desc->n_shapes < 0 || (desc->n_shapes > 0 && !desc->shapes)))
         return fail(plan, GSM_E_INVALID, "shapes missing");
-    const gsm_plan_desc old = plan->desc;
     plan->desc.eps_bg_re = desc->eps_bg_re; plan->desc.eps_bg_im = desc->eps_bg_im;
     plan->desc.eps_b_re = desc->eps_b_re;   plan->desc.eps_b_im = desc->eps_b_im;
     plan->desc.n_shapes = desc->n_shapes;   plan->desc.shapes = desc->shapes;
@@ -636,6 +635,5 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
     }
     plan->desc.shapes = nullptr;          // caller-owned arrays are not retained
     plan->desc.eps_grid_host = nullptr;
-    (void)old;
     return s;
 }
