@@ -248,7 +248,9 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     const int chunk = (int)((d.vlen + cs - 1) / cs);
     const size_t smem = arnoldi_cluster_smem(d, chunk);
     if (smem > 227 * 1024) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the attribute is per function, not per plan: always ask for the device maximum so that plans of different
+    // sizes can coexist
+    cudaError_t e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     if (cs > 8) {
         e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);

@@ -332,3 +332,17 @@ def test_config5b_63cubed_single_solve_satisfies_the_equation():
     c = coeffs(geo)
     _check_equation_rows(geo, c, E.cpu().numpy()[None], kb[None], np.array([TWO_PI]), pol[None], 8)
     plan.close()
+
+
+def test_plans_of_different_sizes_coexist():
+    """Kernel attributes (dynamic shared memory, cluster size) are per function: a small plan created after a large one
+    must not shrink what the large one needs, and vice versa."""
+    big = gsm.plan_from_geometry(wl.woodpile((31, 31, 31)), max_iters=40, max_batch=2)
+    small = gsm.plan_from_geometry(wl.sphere_lattice((7, 7, 7)), max_iters=40, max_batch=2)
+    kb = np.array([[0, 0, 1.35 * TWO_PI], [0, 0, 1.3 * TWO_PI]]); pol = np.zeros((2, 6)); pol[:, 0] = 1.0
+    r1, it1, res1, st1 = big.scan(kb, np.full(2, TWO_PI), pol, tol=1e-8)
+    r2, it2, res2, st2 = small.scan(kb, np.full(2, TWO_PI), pol, tol=1e-8)
+    r3, it3, res3, st3 = big.scan(kb, np.full(2, TWO_PI), pol, tol=1e-8)
+    assert st1 == st2 == st3 == gsm.OK and np.all(res1 <= 1e-7) and np.all(res2 <= 1e-7)
+    assert np.array_equal(r1, r3) and np.array_equal(it1, it3)
+    big.close(); small.close()
