@@ -141,6 +141,19 @@ gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const doubl
 gsm_status gsm_pole_search(int npts, const double* kappa, const double* xi, int Np, int Nd,
                            double kappa_lo, double kappa_hi, double* eta, double* zeta, int* best);
 
+/* Retrieval of one effective index (n_eff = eta / k0, eps_eff = n_eff^2) by the two-stage scan of
+ * DESIGN.md reading R16, all host orchestration around gsm_scan and gsm_pole_search:
+ *   1. coarse scan: ncoarse equidistant kappa = n k0 on [n_lo, n_hi] along the unit direction dir[3] with amplitude pol
+ *      (3 complex), response = component `comp` of the 0-th order field; pole search (Np = 5, Nd = 10) -> estimate eta_c;
+ *   2. fine scan: nfine points with spacing fine_step * k0 centred so that eta_c falls mid-way between the two middle
+ *      nodes (a sample too close to the pole spoils the fit); pole search -> eta.
+ * ncoarse, nfine >= 15 (= Np + Nd); nfine even.  out[0..1] = n_eff (re, im), out[2..3] = eps_eff = n_eff^2,
+ * out[4..5] = pole amplitude zeta.  GSM_NOT_CONVERGED (warning) if a solve hit max_iters; GSM_E_INVALID if no pole with
+ * Re eta inside the scanned window was found in either stage. */
+gsm_status gsm_retrieve_neff(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
+                             double n_lo, double n_hi, int ncoarse, int nfine, double fine_step, double tol,
+                             double out[6]);
+
 /* Text of the last failure on this plan (or of the last failed gsm_plan_create when plan == NULL). */
 const char* gsm_last_error(const gsm_plan* plan);
 

@@ -360,7 +360,12 @@ def pole_search(kappa, xi, Np=5, Nd=10):
             M[s, k] = np.sum(tw**k * xw * w)
         rhs[s] = -np.sum(tw**Np * xw * w)
     scale = np.abs(M).max()
-    p = np.linalg.lstsq(M / scale, rhs / scale, rcond=None)[0]
+    # Eq. 9 is a plain linear system for p_k; solve it in the least-squares sense by QR WITHOUT rank
+    # truncation.  A rank-revealing pseudo-inverse (numpy.linalg.lstsq) returns the minimum-norm solution when the
+    # window sees fewer than Np poles, which makes all Np roots coalesce at the pole and amplifies rounding as
+    # eps^(1/Np); the untruncated solution keeps the true pole as a simple root and lets the spurious ones wander.
+    Q, R = np.linalg.qr(M / scale)
+    p = np.linalg.solve(R, Q.conj().T @ (rhs / scale))
     comp = np.zeros((Np, Np), dtype=np.complex128)               # companion of t^Np + sum p_k t^k
     comp[1:, :-1] = np.eye(Np - 1)
     comp[:, -1] = -p
@@ -473,3 +478,23 @@ def solve_dense_H(D, periods, orders, k_inc, k0, eps_b, pol) -> np.ndarray:
 def solve_gmres_H(D, periods, orders, k_inc, k0, eps_b, pol, tol=1e-13, max_iters=200, matvec=None):
     mv = matvec or toeplitz_matvec
     return gmres(lambda v: apply_operator_H(D, v, periods, k_inc, k0, eps_b, mv), incident(orders, pol), tol, max_iters)
+
+
+def retrieve_two_stage(xi_of_kappa, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, Np=5, Nd=10):
+    """Two-stage retrieval of one effective index (reading R16).
+
+    xi_of_kappa(kappa_array) -> complex responses.  Stage 1: equidistant coarse mesh on [n_lo, n_hi] k0, pole search,
+    estimate eta_c.  Stage 2: nfine (even) points spaced fine_step k0, centred so that eta_c falls mid-way between the
+    two middle nodes, pole search.  Returns (n_eff, eps_eff, zeta)."""
+    coarse = np.linspace(n_lo, n_hi, ncoarse) * k0
+    eta, zeta = pole_search(coarse, xi_of_kappa(coarse), Np, Nd)
+    b = select_pole(eta, zeta, coarse[0], coarse[-1])
+    if b < 0:
+        raise RuntimeError("no pole inside the coarse window")
+    fine = eta[b].real + fine_step * k0 * (np.arange(nfine) - 0.5 * (nfine - 1))
+    eta, zeta = pole_search(fine, xi_of_kappa(fine), Np, Nd)
+    b = select_pole(eta, zeta, fine[0], fine[-1])
+    if b < 0:
+        raise RuntimeError("no pole inside the fine window")
+    n, eps = retrieve_eps(eta[b], k0)
+    return n, eps, zeta[b]

@@ -637,3 +637,52 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
     plan->desc.eps_grid_host = nullptr;
     return s;
 }
+
+
+// ---- retrieval (a10): two-stage scan + pole search -> n_eff, eps_eff -----------------------------------------------
+static gsm_status scan_line(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
+                            const std::vector<double>& kappa, double tol, std::vector<double>& xi, bool* warn) {
+    const int n = (int)kappa.size();
+    std::vector<double> kb(3 * (size_t)n), kk(n, k0), pl(6 * (size_t)n), resp(6 * (size_t)n);
+    for (int i = 0; i < n; ++i) {
+        for (int a = 0; a < 3; ++a) kb[3 * i + a] = kappa[i] * dir[a];
+        for (int q = 0; q < 6; ++q) pl[6 * i + q] = pol[q];
+    }
+    const gsm_status st = gsm_scan(plan, n, kb.data(), kk.data(), pl.data(), tol, resp.data(), nullptr, nullptr, nullptr);
+    if (st < 0) return st;
+    if (st == GSM_NOT_CONVERGED) *warn = true;
+    xi.resize(2 * (size_t)n);
+    for (int i = 0; i < n; ++i) { xi[2 * i] = resp[6 * i + 2 * comp]; xi[2 * i + 1] = resp[6 * i + 2 * comp + 1]; }
+    return GSM_OK;
+}
+
+extern "C" gsm_status gsm_retrieve_neff(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
+                                        double n_lo, double n_hi, int ncoarse, int nfine, double fine_step, double tol,
+                                        double out[6]) {
+    if (!plan) return GSM_E_INVALID;
+    const int Np = 5, Nd = 10;
+    if (!dir || !pol || !out || comp < 0 || comp > 2 || !(k0 > 0.0) || !(n_hi > n_lo) || ncoarse < Np + Nd ||
+        nfine < Np + Nd || (nfine & 1) || !(fine_step > 0.0) || !(tol > 0.0))
+        return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: bad argument");
+    bool warn = false;
+    std::vector<double> kappa(ncoarse), xi;
+    for (int i = 0; i < ncoarse; ++i) kappa[i] = k0 * (n_lo + (n_hi - n_lo) * i / (ncoarse - 1));
+    gsm_status st = scan_line(plan, dir, pol, comp, k0, kappa, tol, xi, &warn);
+    if (st < 0) return st;
+    double eta[2 * Np], zeta[2 * Np];
+    int best = -1;
+    st = gsm_pole_search(ncoarse, kappa.data(), xi.data(), Np, Nd, kappa.front(), kappa.back(), eta, zeta, &best);
+    if (st < 0 || best < 0) return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: no pole inside the coarse window");
+    const double eta_c = eta[2 * best], h = fine_step * k0;
+    kappa.resize(nfine);
+    for (int i = 0; i < nfine; ++i) kappa[i] = eta_c + h * (i - 0.5 * (nfine - 1));   // nfine even: eta_c mid-way
+    st = scan_line(plan, dir, pol, comp, k0, kappa, tol, xi, &warn);
+    if (st < 0) return st;
+    st = gsm_pole_search(nfine, kappa.data(), xi.data(), Np, Nd, kappa.front(), kappa.back(), eta, zeta, &best);
+    if (st < 0 || best < 0) return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: no pole inside the fine window");
+    const double nr = eta[2 * best] / k0, ni = eta[2 * best + 1] / k0;
+    out[0] = nr; out[1] = ni;
+    out[2] = nr * nr - ni * ni; out[3] = 2.0 * nr * ni;
+    out[4] = zeta[2 * best]; out[5] = zeta[2 * best + 1];
+    return warn ? GSM_NOT_CONVERGED : GSM_OK;
+}

@@ -64,6 +64,9 @@ def _load():
     lib.gsm_kernel_class_count.restype = C.c_int
     lib.gsm_kernel_class_name.argtypes = [C.c_int]
     lib.gsm_kernel_class_name.restype = C.c_char_p
+    lib.gsm_retrieve_neff.argtypes = [P, P, P, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
+                                      C.c_double, P]
+    lib.gsm_retrieve_neff.restype = C.c_int
     lib.gsm_last_error.argtypes = [P]
     lib.gsm_last_error.restype = C.c_char_p
     for f in ("gsm_plan_create", "gsm_plan_destroy", "gsm_plan_coeffs", "gsm_plan_info", "gsm_apply", "gsm_solve",
@@ -234,6 +237,20 @@ class Plan:
                                   resp.ctypes.data, iters.ctypes.data, resid.ctypes.data,
                                   fields.data_ptr() if fields is not None else None), self._h)
         return resp, iters, resid, st
+
+
+def _retrieve(self, direction, pol, comp, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):
+    """gsm_retrieve_neff: returns (n_eff, eps_eff, zeta, status) for one (direction, polarisation) pair."""
+    d = _f64(direction, (3,))
+    pl = _f64(np.asarray(pol, dtype=np.complex128).view(np.float64), (6,))
+    out = np.zeros(6)
+    st = _check(_lib.gsm_retrieve_neff(self._h, d.ctypes.data, pl.ctypes.data, int(comp), float(k0), float(n_lo),
+                                       float(n_hi), int(ncoarse), int(nfine), float(fine_step), float(tol),
+                                       out.ctypes.data), self._h)
+    return complex(out[0], out[1]), complex(out[2], out[3]), complex(out[4], out[5]), st
+
+
+Plan.retrieve_neff = _retrieve
 
 
 def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):

@@ -346,3 +346,39 @@ def test_plans_of_different_sizes_coexist():
     assert st1 == st2 == st3 == gsm.OK and np.all(res1 <= 1e-7) and np.all(res2 <= 1e-7)
     assert np.array_equal(r1, r3) and np.array_equal(it1, it3)
     big.close(); small.close()
+
+
+def test_retrieve_neff_config1_vs_oracle_and_survey_value():
+    """gsm_retrieve_neff (two-stage scan + pole search, reading R16) on BASELINE config 1 against the oracle's own
+    two-stage retrieval on dense LU solves, and against the orientation value of SURVEY 8(c) (7^3: 1.0998424676)."""
+    geo = wl.sphere_lattice((7, 7, 7))
+    c = coeffs(geo)
+
+    def xi_oracle(kappa):
+        return np.array([orc.zero_order(orc.solve_dense(c, geo.periods, geo.orders, np.array([0, 0, kv]), TWO_PI,
+                                                        geo.eps_b, [1.0, 0, 0]))[0] for kv in kappa])
+    n_o, eps_o, zeta_o = orc.retrieve_two_stage(xi_oracle, TWO_PI, 1.02, 1.30)
+    plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=32)
+    n_g, eps_g, zeta_g, st = plan.retrieve_neff([0, 0, 1.0], [1.0, 0, 0], 0, TWO_PI, 1.02, 1.30, tol=1e-12)
+    assert st == gsm.OK
+    assert abs(eps_g - eps_o) <= 1e-8 and abs(n_g - n_o) <= 1e-8
+    assert abs(zeta_g - zeta_o) <= 1e-6 * abs(zeta_o)
+    assert abs(n_g.real - 1.0998424676) <= 1e-8 and abs(n_g.imag) <= 1e-9
+    with pytest.raises(gsm.GsmError):          # an odd fine mesh would put a node on the estimate: rejected
+        plan.retrieve_neff([0, 0, 1.0], [1.0, 0, 0], 0, TWO_PI, 1.02, 1.30, nfine=17, tol=1e-10)
+    plan.close()
+
+
+def test_retrieve_neff_config3_tensor_entries():
+    """BASELINE config 3: the three diagonal entries of eps_eff (reading R14) at 15^3 orders against the orientation
+    values of SURVEY 8(c): n = 1.11151881 (z,x), 1.09189330 (x,y), 1.06709104 (y,z)."""
+    geo = wl.ellipsoid_lattice((15, 15, 15))
+    plan = gsm.plan_from_geometry(geo, max_iters=120, max_batch=32)
+    expect = {"xx": 1.11151881, "yy": 1.09189330, "zz": 1.06709104}
+    for key, (pa, qa) in wl.DIRECTIONS.items():
+        d = np.zeros(3); d[pa] = 1.0
+        pol = np.zeros(3, dtype=complex); pol[qa] = 1.0
+        n, eps, zeta, st = plan.retrieve_neff(d, pol, qa, TWO_PI, 1.02, 1.30, tol=1e-11)
+        assert st == gsm.OK and abs(n.real - expect[key]) <= 2e-8 and abs(n.imag) <= 1e-8
+        assert abs(eps - n * n) <= 1e-14
+    plan.close()
