@@ -322,3 +322,27 @@ def test_laminate_long_wavelength_limits():
         errs.append(abs(eta.real - btm) / k0)
     assert errs[0] > errs[1] > errs[2]
     assert 1.6 < errs[0] / errs[1] < 2.6 and 1.6 < errs[1] / errs[2] < 2.6   # ~1/N
+
+
+def test_two_stage_retrieval_synthetic_pole_and_uniform_cell():
+    """retrieve_two_stage (reading R16) recovers a known pole of a synthetic meromorphic response, and for the uniform
+    cell (closed form: pole at kappa = k0 sqrt(eps_2)) returns n_eff = sqrt(eps_2), eps_eff = eps_2."""
+    import numpy as np
+    from oracle import gsm_oracle as orc
+    k0 = 2.0 * np.pi
+    eta_true, zeta_true = 1.2345678 * k0 + 0.0j, 0.37 - 0.11j
+
+    def xi(kappa):
+        return zeta_true / (kappa - eta_true) + 0.3 - 0.02 * kappa + 0.004 * kappa**2 + 0.05 / (kappa + 9.0)
+    n, eps, zeta = orc.retrieve_two_stage(xi, k0, 1.05, 1.45)
+    assert abs(n - 1.2345678) <= 1e-11 and abs(eps - 1.2345678**2) <= 1e-10 and abs(zeta - zeta_true) <= 1e-8
+
+    eps2 = 2.5
+    shapes = [dict(kind=orc.BOX, center=(0, 0, 0), size=(0.2, 0.2, 0.2), eps=eps2)]
+    c = orc.coeffs_analytic((0.2, 0.2, 0.2), (3, 3, 3), shapes, 1.0, 1.0)
+
+    def xi_cell(kappa):
+        return np.array([orc.zero_order(orc.solve_dense(c, (0.2, 0.2, 0.2), (3, 3, 3), np.array([0, 0, kv]), k0, 1.0,
+                                                        [1.0, 0, 0]))[0] for kv in kappa])
+    n, eps, _ = orc.retrieve_two_stage(xi_cell, k0, 1.3, 1.8)
+    assert abs(eps - eps2) <= 1e-9 and abs(n - np.sqrt(eps2)) <= 1e-9
