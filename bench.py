@@ -54,13 +54,16 @@ def _peaks():
 
 def _traffic(kernel, alg_bytes_per_launch):
     """DRAM bytes per launch of `kernel`: the dram/algorithmic ratio of the committed ncu --set full capture
-    (profiles/ncu_traffic.json) scaled to the average launch of the timed region; None if that kernel was not captured."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    (profiles/ncu_traffic.csv) scaled to the average launch of the timed region; None if that kernel was not captured."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
         return None
     with open(path) as f:
-        ratio = json.load(f).get(kernel, {}).get("ratio")
-    return None if ratio is None else ratio * alg_bytes_per_launch
+        rows = [line.strip().split(",") for line in f if line.strip()]
+    for r in rows[1:]:
+        if r[0] == kernel:
+            return float(r[rows[0].index("ratio")]) * alg_bytes_per_launch
+    return None
 
 
 class ClockSampler:
