@@ -30,26 +30,15 @@ class Geometry:
     eps_bg: complex = 1.0
     eps_b: complex = 1.0
     voxels: np.ndarray | None = None               # complex128 [Nv1, Nv2, Nv3], i3 fastest
-    fft_grid: tuple = ()
+    fft_grid: tuple = ()                           # unused placeholder (the FFT grid is the library's choice: Plan.info())
 
     @property
     def n(self) -> int:
         return int(np.prod(self.orders))
 
 
-def fft_size(N: int) -> int:
-    """Smallest power of two >= 2N-1 (1 if N == 1) - reading R2."""
-    if N == 1:
-        return 1
-    p = 1
-    while p < 2 * N - 1:
-        p *= 2
-    return p
-
-
 def _geo(name, periods, orders, shapes=None, eps_bg=1.0, eps_b=1.0, voxels=None) -> Geometry:
-    return Geometry(name, tuple(periods), tuple(orders), shapes or [], eps_bg, eps_b, voxels,
-                    tuple(fft_size(N) for N in orders))
+    return Geometry(name, tuple(periods), tuple(orders), shapes or [], eps_bg, eps_b, voxels, ())
 
 
 def sphere_lattice(orders=(7, 7, 7), period=0.2, radius_frac=0.3, eps=4.0, eps_bg=1.0) -> Geometry:
