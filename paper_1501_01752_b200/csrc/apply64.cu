@@ -18,7 +18,7 @@
 namespace gsm {
 
 // ------------------------------------------------------------------------------------------- pass 2, P1 = P2 = 64
-// One CTA per (solve b, component c, z-position pos3) plane, 8 warps.  A[r][col]: row r = y-position (64), 32 columns
+// One CTA per (solve b, z-position pos3), 8 warps, the three component planes in turn.  A[r][col]: row r = y-position (64), 32 columns
 // = x-index i1 rotated by r/8, so that both the y-phase (lanes differ in u = r/8) and the x-phase (lanes differ in
 // i1) touch 8 distinct 16-byte bank groups per quarter-warp.
 //   y forward : group (i1 = 4 warp + ln) reads its 4 x 8 inputs straight from W (contiguous in i2), writes rows of A
@@ -32,7 +32,9 @@ namespace gsm {
 __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, cplx* __restrict__ W,
                                                            const cplx* __restrict__ chat64,
                                                            const int* __restrict__ active) {
-    const int b = blockIdx.z, c = blockIdx.y, pos3 = blockIdx.x;
+    // one CTA per (solve b, z-position pos3); the three components are done in turn, the inputs of the next component
+    // being fetched from W while the current one is transformed
+    const int b = blockIdx.y, pos3 = blockIdx.x;
     if (active && !active[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* A = reinterpret_cast<cplx*>(smem_raw);   // [64][32]
@@ -42,56 +44,68 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
     cplx tw[7];
     load_group_twiddles(tw, g.tw[0], u);
     cplx* sc = scratch + (warp * 4 + ln) * SC_LINE;
-    cplx* Wp = W + (((long)b * 3 + c) * 64 + pos3) * g.NL;
-    cplx a[8];
-
-    {   // ---- y forward
-        const int i1 = warp * 4 + ln;
+    const long cstride = 64L * g.NL;
+    cplx* Wp = W + ((long)b * 3 * 64 + pos3) * g.NL;   // component 0; component c at + c * cstride
+    const int i1y = warp * 4 + ln;                      // y-phase line of this group
+    cplx a[8], nx[4];
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const int i2 = u + 8 * p;
-            a[p] = (i1 < N1 && i2 < N2) ? Wp[i1 * N2 + i2] : make_double2(0.0, 0.0);
-        }
-        fwd64_group(a, tw, sc, u);
-        const int col = (i1 + u) & 31;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) A[(8 * u + q) * 32 + col] = a[q];
+    for (int p = 0; p < 4; ++p) {
+        const int i2 = u + 8 * p;
+        nx[p] = (i1y < N1 && i2 < N2) ? Wp[i1y * N2 + i2] : make_double2(0.0, 0.0);
     }
-    __syncthreads();
-    // ---- x: forward, multiply by the coefficient spectrum, inverse
 #pragma unroll 1
-    for (int round = 0; round < 2; ++round) {
-        const int r = (round * 8 + warp) * 4 + ln;
-        cplx* Ar = A + r * 32;
-        const int rot = r >> 3;
+    for (int c = 0; c < 3; ++c, Wp += cstride) {
+        {   // ---- y forward
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const int i1 = u + 8 * p;
-            a[p] = (i1 < N1) ? Ar[(i1 + rot) & 31] : make_double2(0.0, 0.0);
+            for (int p = 0; p < 4; ++p) a[p] = nx[p];
+            if (c < 2) {
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    const int i2 = u + 8 * p;
+                    nx[p] = (i1y < N1 && i2 < N2) ? Wp[cstride + i1y * N2 + i2] : make_double2(0.0, 0.0);
+                }
+            }
+            fwd64_group(a, tw, sc, u);
+            const int col = (i1y + u) & 31;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) A[(8 * u + q) * 32 + col] = a[q];
         }
-        const cplx* cp = chat64 + ((long)(pos3 * 64 + r) * 64) + u;
-        fwd64_group(a, tw, sc, u);
+        __syncthreads();
+        // ---- x: forward, multiply by the coefficient spectrum, inverse
+#pragma unroll 1
+        for (int round = 0; round < 2; ++round) {
+            const int r = (round * 8 + warp) * 4 + ln;
+            cplx* Ar = A + r * 32;
+            const int rot = r >> 3;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], __ldg(cp + 8 * q));
-        inv64_group(a, tw, sc, u);
+            for (int p = 0; p < 4; ++p) {
+                const int i1 = u + 8 * p;
+                a[p] = (i1 < N1) ? Ar[(i1 + rot) & 31] : make_double2(0.0, 0.0);
+            }
+            const cplx* cp = chat64 + ((long)(pos3 * 64 + r) * 64) + u;
+            fwd64_group(a, tw, sc, u);
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const int i1 = u + 8 * p;
-            if (i1 < N1) Ar[(i1 + rot) & 31] = a[p];
+            for (int q = 0; q < 8; ++q) a[q] = cmul(a[q], __ldg(cp + 8 * q));
+            inv64_group(a, tw, sc, u);
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                const int i1 = u + 8 * p;
+                if (i1 < N1) Ar[(i1 + rot) & 31] = a[p];
+            }
         }
-    }
-    __syncthreads();
-    {   // ---- y inverse
-        const int i1 = warp * 4 + ln;
-        const int col = (i1 + u) & 31;
+        __syncthreads();
+        {   // ---- y inverse
+            const int col = (i1y + u) & 31;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) a[q] = A[(8 * u + q) * 32 + col];
-        inv64_group(a, tw, sc, u);
+            for (int q = 0; q < 8; ++q) a[q] = A[(8 * u + q) * 32 + col];
+            inv64_group(a, tw, sc, u);
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            const int i2 = u + 8 * p;
-            if (i1 < N1 && i2 < N2) Wp[i1 * N2 + i2] = a[p];
+            for (int p = 0; p < 4; ++p) {
+                const int i2 = u + 8 * p;
+                if (i1y < N1 && i2 < N2) Wp[i1y * N2 + i2] = a[p];
+            }
         }
+        __syncthreads();   // A is rewritten by the next component's y-forward
     }
 }
 
@@ -275,7 +289,7 @@ cudaError_t launch_chat64_layout(const cplx* d_chat, cplx* d_chat64, cudaStream_
 }
 cudaError_t launch_xy_conv64(const ApplyGeom& g, int batch, cplx* d_W, const cplx* d_chat64, const int* d_active,
                              cudaStream_t st) {
-    xy_conv64_kernel<<<dim3(64, 3, batch), 256, XY64_SMEM, st>>>(g, d_W, d_chat64, d_active);
+    xy_conv64_kernel<<<dim3(64, batch), 256, XY64_SMEM, st>>>(g, d_W, d_chat64, d_active);
     return cudaGetLastError();
 }
 static const size_t ZF64_SMEM = sizeof(cplx) * (32 * SC_LINE);   // >= 64 * 32 tile
