@@ -87,8 +87,7 @@ def _f64(a, shape=None):
 
 def _check(status, plan=None, allow_warning=True):
     if status < 0 or (status > 0 and not allow_warning):
-        msg = _lib.gsm_last_error(plan).decode() if True else ""
-        raise GsmError(status, msg)
+        raise GsmError(status, _lib.gsm_last_error(plan).decode())
     return status
 
 
@@ -239,18 +238,15 @@ class Plan:
         return resp, iters, resid, st
 
 
-def _retrieve(self, direction, pol, comp, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):
-    """gsm_retrieve_neff: returns (n_eff, eps_eff, zeta, status) for one (direction, polarisation) pair."""
-    d = _f64(direction, (3,))
-    pl = _f64(np.asarray(pol, dtype=np.complex128).view(np.float64), (6,))
-    out = np.zeros(6)
-    st = _check(_lib.gsm_retrieve_neff(self._h, d.ctypes.data, pl.ctypes.data, int(comp), float(k0), float(n_lo),
-                                       float(n_hi), int(ncoarse), int(nfine), float(fine_step), float(tol),
-                                       out.ctypes.data), self._h)
-    return complex(out[0], out[1]), complex(out[2], out[3]), complex(out[4], out[5]), st
-
-
-Plan.retrieve_neff = _retrieve
+    def retrieve_neff(self, direction, pol, comp, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):
+        """gsm_retrieve_neff: returns (n_eff, eps_eff, zeta, status) for one (direction, polarisation) pair."""
+        d = _f64(direction, (3,))
+        pl = _f64(np.asarray(pol, dtype=np.complex128).view(np.float64), (6,))
+        out = np.zeros(6)
+        st = _check(_lib.gsm_retrieve_neff(self._h, d.ctypes.data, pl.ctypes.data, int(comp), float(k0), float(n_lo),
+                                           float(n_hi), int(ncoarse), int(nfine), float(fine_step), float(tol),
+                                           out.ctypes.data), self._h)
+        return complex(out[0], out[1]), complex(out[2], out[3]), complex(out[4], out[5]), st
 
 
 def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):
