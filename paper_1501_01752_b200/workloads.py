@@ -130,6 +130,19 @@ def scan_points(kappa, prop_axis, pol_axis, k0=TWO_PI):
     return kb, np.full(len(kappa), float(k0)), pol
 
 
+def direction_sweep(count, seed=SEED):
+    """Direction sweep at fixed omega: `count` seeded unit vectors s and, for each,
+    the transverse unit amplitude a = s x z / |s x z|.  Returns a list of (s[3], a[3])."""
+    rng = np.random.default_rng(seed + 4)
+    out = []
+    for _ in range(count):
+        v = rng.standard_normal(3)
+        s = v / np.linalg.norm(v)
+        a = np.cross(s, [0.0, 0.0, 1.0])
+        out.append((s, a / np.linalg.norm(a)))
+    return out
+
+
 def random_field(batch, orders, seed=SEED) -> np.ndarray:
     """Seeded complex standard-normal x[batch, 3, N1, N2, N3] for operator-apply tests."""
     rng = np.random.default_rng(seed)

@@ -85,6 +85,43 @@ def test_eps_b_offset_term():
     assert np.allclose(c2, ref, atol=1e-15)
 
 
+def test_ellipsoid_coefficients_pinned():
+    """ELLIPSOID branch of coeffs_analytic (config 3 rests on it), pinned four ways:
+    (1) radial quadrature: the affine map r = s o u turns the ellipsoid into the unit ball, so
+        c_d = Delta (4 pi a b c / V) int_0^1 u^2 sinc(|G o s| u) du exp(-i G.r_c) - independent of the closed form;
+    (2) direct DFT of a voxelised off-centre ellipsoid converges to it as the grid refines;
+    (3) a = b = c reduces to the sphere coefficients; (4) c_0 = f Delta with f = 4 pi a b c / (3 V)."""
+    per, orders = (0.2, 0.25, 0.3), (3, 3, 3)
+    semi, ctr, eps_i = (0.07, 0.05, 0.04), (0.03, -0.02, 0.05), 12.0
+    sh = [dict(kind=W.ELLIPSOID, center=ctr, size=semi, eps=eps_i)]
+    c = O.coeffs_analytic(per, orders, sh, 1.0, 1.0)
+    V = per[0] * per[1] * per[2]
+    delta = eps_i - 1.0
+    for d in itertools.product(range(-2, 3), repeat=3):
+        G = [2 * np.pi * d[a] / per[a] for a in range(3)]
+        x = math.sqrt(sum((G[a] * semi[a]) ** 2 for a in range(3)))
+        val, _ = scipy.integrate.quad(lambda u: u * u * np.sinc(x * u / np.pi), 0, 1, epsabs=1e-15, epsrel=1e-13)
+        ref = delta * 4 * np.pi * semi[0] * semi[1] * semi[2] * val / V * np.exp(-1j * sum(G[a] * ctr[a] for a in range(3)))
+        assert abs(c[d[0] + 2, d[1] + 2, d[2] + 2] - ref) < 1e-13
+    assert abs(c[2, 2, 2] - delta * 4 / 3 * np.pi * semi[0] * semi[1] * semi[2] / V) < 1e-15
+    assert np.allclose(c, np.conj(c[::-1, ::-1, ::-1]), atol=1e-16)
+    errs = []
+    for nv in (16, 48, 96):
+        ax = [np.arange(nv) * per[a] / nv for a in range(3)]
+        dd = []
+        for a in range(3):
+            t = (ax[a] - ctr[a] + per[a] / 2) % per[a] - per[a] / 2          # minimum-image offset from the centre
+            dd.append((t / semi[a]) ** 2)
+        inside = dd[0][:, None, None] + dd[1][None, :, None] + dd[2][None, None, :] <= 1.0
+        cv = O.coeffs_voxel(np.where(inside, eps_i, 1.0), orders, 1.0)
+        errs.append(np.abs(cv - c).max())
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 5e-3 * abs(c[2, 2, 2])
+    R = 0.06
+    cs = O.coeffs_analytic(per, orders, [dict(kind=W.SPHERE, center=ctr, size=(R, 0, 0), eps=eps_i)], 1.0, 1.0)
+    ce = O.coeffs_analytic(per, orders, [dict(kind=W.ELLIPSOID, center=ctr, size=(R, R, R), eps=eps_i)], 1.0, 1.0)
+    assert np.max(np.abs(cs - ce)) < 1e-15                     # same numbers up to the rounding of |G| R vs |G o s|
+
+
 def test_voxel_dft_separable_vs_literal_triple_sum():
     rng = np.random.default_rng(3)
     grid = rng.uniform(1, 5, (4, 5, 6)) + 1j * rng.uniform(0, 1, (4, 5, 6))
