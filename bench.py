@@ -7,15 +7,21 @@ at 31^3 orders; % of the HBM roofline).
 Workload (BASELINE.json config 5a; recipe in DESIGN.md "Input recipe"): random voxel composite
 (20 seeded spheres on a 128^3 voxel grid, cubic Lambda = 0.25 lambda), 31^3 Fourier orders (FFT grid 64^3), 256
 concurrent (k, omega) solves per GPU: kappa equidistant on n in [1.05, 1.20], k || z, a = x, GMRES tol 1e-10.
-One step = one pass of the whole hot path over that batch: gsm_scan of the 256 points (operator applies, Arnoldi /
-Gram-Schmidt, least squares, update, true residual, 0-th order response).  Inputs: the per-step working set is
+One step = one pass of the whole hot path over that batch: a scan of the 256 points (operator applies, Arnoldi /
+Gram-Schmidt, least squares, update, true residual, 0-th order response).  The points form the equidistant kappa mesh
+of the method, so the scan runs as gsm_scan_mesh: 5 coarse-to-fine waves (16 + 16 + 32 + 64 + 128
+solves), each started from the (pole-aware) interpolation of the earlier solutions; every point is solved to the same
+tolerance and its true residual is checked with one more operator apply.  The plain
+lock-step gsm_scan (all 256 from a zero start) is timed beside it (`lockstep_zero_start`).  Inputs: the per-step working set is
 ~24 GB of Krylov basis, far above the 126 MB L2, so no L2 flush is needed between timed iterations.
 
-Prints ONE JSON line (rank 0).  `value`: plan resident on the device (coefficient spectrum built).  `e2e`: per step
-the voxel grid is uploaded from pinned host memory and step a0 re-run (gsm_plan_set_cell), then the scan, the
-device->host read of the responses, and the host pole search.  `roofline`: dominant kernel class, timed live with CUDA
-events on the plan's stream inside the timed region (gsm_plan_profile).  `cpu_baseline`: the CPU oracle as it stands
-(O(n^2) Toeplitz product + full GMRES) on one of the 256 points.
+Prints ONE JSON line (rank 0).  `value`: plan resident on the device (coefficient spectrum built), per-launch
+profiling OFF.  `e2e`: per step the voxel grid is uploaded from pinned host memory and step a0 re-run
+(gsm_plan_set_cell), then the scan (through scan_shard.sharded_scan: this rank's block of the list, host-side gather),
+the device->host read of the responses, and the host pole search.  `roofline` / `kernel_ms_per_step`: a SECOND pass of
+the same K steps with every launch bracketed by CUDA events on the plan's stream (gsm_plan_profile); algorithmic bytes
+are billed from the final iteration counts of every solve.  `cpu_baseline`: the CPU oracle as it stands (O(n^2)
+Toeplitz product + full GMRES) on one of the 256 points, plus one operator apply (the metric's other half).
 
 --impl reference: the oracle itself on the host cores, one solve (one point of the scan) per step.
 """
@@ -40,6 +46,7 @@ ORDERS = (31, 31, 31)
 BATCH = 256
 TOL = 1e-10
 MAX_ITERS = 64
+LEVELS = 5          # gsm_scan_mesh waves (1 = plain gsm_scan)
 N_LO, N_HI = 1.05, 1.20
 TWO_PI = 2.0 * np.pi
 
@@ -53,17 +60,22 @@ def _peaks():
 
 
 def _traffic(kernel, alg_bytes_per_launch):
-    """DRAM bytes per launch of `kernel`: the dram/algorithmic ratio of the committed ncu --set full capture
-    (profiles/ncu_traffic.csv) scaled to the average launch of the timed region; None if that kernel was not captured."""
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` capture (profiles/ncu_traffic.csv: one row
+    per captured launch - first, middle and late iterations - with its dram__bytes_read+write and its algorithmic bytes):
+    (sum of captured DRAM bytes / sum of their algorithmic bytes) x this run's average algorithmic bytes per launch.
+    None if that kernel was not captured."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
         return None
     with open(path) as f:
-        rows = [line.strip().split(",") for line in f if line.strip()]
+        rows = [line.strip().split(",") for line in f if line.strip() and not line.startswith("#")]
+    hdr = rows[0]
+    dram = alg = 0.0
     for r in rows[1:]:
-        if r[0] == kernel:
-            return float(r[rows[0].index("ratio")]) * alg_bytes_per_launch
-    return None
+        if r[hdr.index("kernel")] == kernel:
+            dram += float(r[hdr.index("dram_bytes")])
+            alg += float(r[hdr.index("algorithmic_bytes")])
+    return dram / alg * alg_bytes_per_launch if alg > 0 else None
 
 
 class ClockSampler:
@@ -118,6 +130,14 @@ def workload(rank, world):
     return geo, kappa, kb, k0, pol
 
 
+def host_cores():
+    """Threads the oracle's OpenMP loop can use: the affinity mask of this process."""
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
 def oracle_solve_once(geo, kb, k0, pol):
     """One solve by the CPU oracle as it stands; returns (seconds, iterations, threads)."""
     from oracle import gsm_oracle as orc
@@ -125,7 +145,20 @@ def oracle_solve_once(geo, kb, k0, pol):
     t0 = time.perf_counter()
     _, hist, iters = orc.solve_gmres(c, geo.periods, geo.orders, kb, float(k0), geo.eps_b, pol[0::2] + 1j * pol[1::2],
                                      tol=TOL, max_iters=MAX_ITERS, matvec=orc.toeplitz_matvec_c)
-    return time.perf_counter() - t0, iters, orc.num_threads()
+    return time.perf_counter() - t0, iters, min(orc.num_threads(), host_cores())
+
+
+def oracle_apply_once(geo, kb, k0, reps=3):
+    """Operator applies by the CPU oracle as it stands (O(n^2) Toeplitz product + Green dyadic); seconds per apply."""
+    from oracle import gsm_oracle as orc
+    from paper_1501_01752_b200 import workloads as wl
+    c = orc.coeffs_voxel(geo.voxels, geo.orders, geo.eps_b)
+    x = wl.random_field(1, geo.orders)[0]
+    orc.apply_operator(c, x, geo.periods, kb, float(k0), geo.eps_b, orc.toeplitz_matvec_c)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        orc.apply_operator(c, x, geo.periods, kb, float(k0), geo.eps_b, orc.toeplitz_matvec_c)
+    return (time.perf_counter() - t0) / reps
 
 
 def run_reference(args):
@@ -180,7 +213,7 @@ def run_gsm(args):
 
     geo, kappa, kb, k0, pol = workload(rank, world)
     stream = torch.cuda.Stream()
-    plan = gsm.plan_from_geometry(geo, max_iters=MAX_ITERS, max_batch=BATCH, stream=stream)
+    plan = gsm.plan_from_geometry(geo, max_iters=MAX_ITERS, max_batch=BATCH, stream=stream, flags=args.flags)
     pinned_grid = torch.from_numpy(geo.voxels).pin_memory()
 
     def barrier():
@@ -197,22 +230,27 @@ def run_gsm(args):
         return float(t.item())
 
     def step():
-        return plan.scan(kb, k0, pol, tol=TOL)
+        return plan.scan(kb, k0, pol, tol=TOL, levels=args.levels)
+
+    from paper_1501_01752_b200 import scan_shard, workloads as wl
+    kappa_all = wl.kappa_mesh(N_LO, N_HI, BATCH * world)
+    kb_all, k0_all, pol_all = wl.scan_points(kappa_all, 2, 0)
 
     def step_e2e():
+        """What a user of the library runs: new cell -> a0, this rank's block of the scan list, gather, pole search."""
         plan.set_cell(geo.periods, eps_bg=geo.eps_bg, eps_b=geo.eps_b, voxels=pinned_grid)
-        resp, iters, resid, st = plan.scan(kb, k0, pol, tol=TOL)
-        eta, zeta, best = gsm.pole_search(kappa, resp[:, 0], 5, 10)
-        return resp, iters, resid, st, (eta[best] if best >= 0 else None)
+        resp, iters, resid = scan_shard.sharded_scan(lambda a, b, c: plan.scan(a, b, c, tol=TOL, levels=args.levels)[:3],
+                                                     kb_all, k0_all, pol_all, rank, world)
+        eta, zeta, best = gsm.pole_search(kappa_all, resp[:, 0], 5, 10)
+        return resp, iters, resid, (eta[best] if best >= 0 else None)
 
     for _ in range(args.warmup):
         resp, iters, resid, st = step()
     assert st >= 0 and float(np.max(resid)) <= 1e-9, f"solve failed: status {st}, max residual {np.max(resid):.2e}"
 
-    # ---- device-resident timed region --------------------------------------------------------------------------
+    # ---- device-resident timed region (per-launch profiling off) ---------------------------------------------------
     sampler = ClockSampler(local)
-    plan.profile(True)
-    plan.profile_read(reset=True)
+    plan.profile(False)
     barrier()
     if rank == 0:
         sampler.start()
@@ -224,9 +262,32 @@ def run_gsm(args):
     barrier()
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     clocks = sampler.stop() if rank == 0 else None
+    value = BATCH * world * args.steps / (ms_total * 1e-3)
+
+    # ---- the plain lock-step scan (all points from a zero start), for comparison ----------------------------------------
+    plan.scan(kb, k0, pol, tol=TOL)
+    barrier()
+    z0, z1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    z0.record(stream)
+    for _ in range(2):
+        _, z_iters, z_resid, _ = plan.scan(kb, k0, pol, tol=TOL)
+    z1.record(stream)
+    barrier()
+    z_ms = max_over_ranks(z0.elapsed_time(z1)) / 2
+
+    # ---- second pass, same steps, every launch bracketed by CUDA events: the kernel split and the roofline ---------
+    plan.profile(True)
+    plan.profile_read(reset=True)
+    barrier()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    for _ in range(args.steps):
+        step()
+    p1.record(stream)
+    barrier()
+    ms_profiled = p0.elapsed_time(p1)
     prof = plan.profile_read(reset=True)
     plan.profile(False)
-    value = BATCH * world * args.steps / (ms_total * 1e-3)
 
     # ---- end to end through the C ABI with host buffers ---------------------------------------------------------
     for _ in range(min(args.warmup, 2)):
@@ -239,21 +300,22 @@ def run_gsm(args):
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e_value = BATCH * world * args.steps / e2e_s
     h2d = int(pinned_grid.numel() * 16 + kb.nbytes + k0.nbytes + pol.nbytes + 16)
-    d2h = int(resp.nbytes + iters.nbytes + resid.nbytes + 4 * int(np.max(iters)))   # + nactive read per iteration
+    d2h = int(resp.nbytes + iters.nbytes + resid.nbytes + 4 * BATCH + 4 * int(np.max(iters)))   # + active flags, nactive per iteration
 
     # ---- operator applies/s (the other half of BASELINE.json's metric) -------------------------------------------
     x = torch.randn((BATCH, 3) + ORDERS, dtype=torch.complex128, device="cuda")
     y = torch.empty_like(x)
     torch.cuda.synchronize()
-    for _ in range(3):
-        plan.apply(kb, k0, x, out=y)
     a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     napply = 20
-    barrier()
-    a0.record(stream)
-    for _ in range(napply):
-        plan.apply(kb, k0, x, out=y)
-    a1.record(stream)
+    with torch.cuda.stream(stream):       # the plan's stream is torch's current stream: no cross-stream ordering needed
+        for _ in range(3):
+            plan.apply(kb, k0, x, out=y)
+        barrier()
+        a0.record(stream)
+        for _ in range(napply):
+            plan.apply(kb, k0, x, out=y)
+        a1.record(stream)
     barrier()
     apply_ms = max_over_ranks(a0.elapsed_time(a1)) / napply
     V = 16.0 * 3 * geo.n
@@ -329,17 +391,26 @@ def run_gsm(args):
     gpu_launches = int(sum(v[0] for v in timed.values()))
     mean_it = float(np.mean(iters))
     # whole-step figure against SURVEY 8(d)'s B_solve = (m(m+1)/2 + 3m + 1) V + m |Chat| per solve
-    b_solve = float(np.sum((iters * (iters + 1.0) / 2 + 3.0 * iters + 1.0) * V)) + float(np.max(iters)) * chat_bytes
+    # (+ 3 V for a solve started from a guess: the apply that forms r0 = b - A x0 and the read of x0 in the update)
+    guessed = BATCH - len(range(0, BATCH, 1 << (args.levels - 1))) if args.levels > 1 else 0
+    wave0 = np.arange(BATCH) % (1 << (args.levels - 1)) == 0
+    b_solve = (float(np.sum((iters * (iters + 1.0) / 2 + 3.0 * iters + 1.0) * V)) + 3.0 * V * guessed
+               + float(np.sum(iters)) / BATCH * chat_bytes)
     path_gbs = b_solve * args.steps / (ms_total * 1e-3) / 1e9
 
     # ---- CPU oracle on a bounded sample ---------------------------------------------------------------------------
     cpu_t, cpu_it, cores = oracle_solve_once(geo, kb[0], k0[0], pol[0])
+    cpu_apply_t = oracle_apply_once(geo, kb[0], k0[0])
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD_NAME, "orders": list(ORDERS), "fft_grid": fft_grid,
                    "batch_per_gpu": BATCH, "tol": TOL, "max_iters": MAX_ITERS, "mean_iters": mean_it,
+                   "scan_driver": (f"gsm_scan_mesh, {args.levels} coarse-to-fine waves with interpolated initial guesses "
+                                   "(PAPER.md:101 equidistant mesh)" if args.levels > 1 else "gsm_scan, zero start"),
+                   "mean_iters_zero_start_wave": float(np.mean(iters[wave0])),
+                   "mean_iters_guessed_waves": float(np.mean(iters[~wave0])) if guessed else None,
                    "max_true_resid": float(np.max(resid)), "parallelism": f"scan list sharded over {world} GPU(s), no collective",
                    "l2": "working set per step ~24 GB >> 126 MB L2; no flush needed"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -351,51 +422,31 @@ def run_gsm(args):
                      "launches": n_l, "avg_launch_ms": ms_l / n_l, "algorithmic_bytes_per_launch": by_l / n_l,
                      "share_of_step": ms_l / kernels_ms},
         "path_roofline": {"algorithmic_GBps": path_gbs, "frac": path_gbs / peak,
-                          "definition": "SURVEY 8(d) B_solve summed over the batch / step time"},
+                          "definition": "SURVEY 8(d) B_solve summed over the batch / step time (profiling off)"},
+        "profiled_pass": {"ms_per_step": ms_profiled / args.steps,
+                          "note": "second pass of the same steps with a CUDA event pair around every launch; "
+                                  "roofline, kernel_ms_per_step and kernel_GBps come from it, value and e2e do not"},
         "kernel_ms_per_step": {k: v[1] / args.steps for k, v in timed.items()},
         "kernel_GBps": {k: (v[2] / (v[1] * 1e-3) / 1e9 if v[1] > 0 and v[2] > 0 else None) for k, v in timed.items()},
         "applies_per_s": BATCH * world / (apply_ms * 1e-3),
         "apply": {"ms_per_batch_apply": apply_ms, "algorithmic_GBps": apply_alg_bytes / (apply_ms * 1e-3) / 1e9,
                   "frac": apply_alg_bytes / (apply_ms * 1e-3) / 1e9 / peak, "definition": "(2V x 256 + |Chat|) / time"},
+        "lockstep_zero_start": {"value": BATCH * world / (z_ms * 1e-3), "unit": UNIT, "ms_per_step": z_ms,
+                                "mean_iters": float(np.mean(z_iters)), "max_true_resid": float(np.max(z_resid)),
+                                "note": "plain gsm_scan: all 256 points in one lock-step batch from x0 = 0"},
         "h_form": {"value": BATCH / (h_ms * 1e-3), "unit": UNIT, "ms_per_step": h_ms, "mean_iters": float(np.mean(h_iters)),
                    "max_true_resid": float(np.max(h_resid)), "note": "same workload, Eq. 5 (H-field) formulation, this rank only"},
         "config5b_63cubed": c5b,
         "cpu_baseline": {"value": 1.0 / cpu_t, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": f"1 of the {BATCH} (k,omega) points (full GMRES solve with the O(n^2) Toeplitz product, "
-                                   f"{cpu_it} iterations, {cpu_t:.1f} s)"},
+                                   f"{cpu_it} iterations, {cpu_t:.1f} s)",
+                         "applies_per_s": 1.0 / cpu_apply_t,
+                         "apply_sample": f"one operator apply at 31^3 orders (O(n^2) Toeplitz product + Green dyadic), "
+                                         f"mean of 3, {cpu_apply_t:.2f} s"},
     }
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-
-
-def run_table1(args):
-    """Context only: single-solve times on the shape of the paper's Table 1 (lattice of spheres with
-    refractive index 3 in air, GMRES to 1e-8; radius, period and wavevector are not printed - here R = 0.3 Lambda,
-    Lambda = 0.3 lambda, k = 1.3 k0 z, a = x) at the orders this build supports (16^3, 32^3, 64^3)."""
-    import torch
-    import __graft_entry__ as ge
-    ge.build()
-    from paper_1501_01752_b200 import gsm, workloads as wl
-    paper_gpu_s = {16: 0.166, 32: 0.244, 64: 0.448}            # GeForce GTX Titan, PAPER.md:111-115
-    paper_cpu_s = {16: 0.515, 32: 4.204, 64: 39.047}           # Xeon E5640
-    rows = []
-    for N in (16, 32, 64):
-        geo = wl.sphere_lattice((N, N, N), period=0.3, radius_frac=0.3, eps=9.0)
-        plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=1)
-        kb, pol = np.array([0.0, 0.0, 1.3 * TWO_PI]), np.array([1.0, 0, 0], dtype=complex)
-        plan.solve(kb, TWO_PI, pol, tol=1e-8)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(10):                                      # the paper averages 10 runs
-            _, _, it, res, st = plan.solve(kb, TWO_PI, pol, tol=1e-8)
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / 10
-        rows.append({"orders": N, "solve_s": dt, "iters": int(it), "true_resid": float(res), "status": int(st),
-                     "paper_gtx_titan_s": paper_gpu_s[N], "paper_xeon_e5640_s": paper_cpu_s[N]})
-        plan.close()
-    print(json.dumps({"table1_context": rows, "note": "geometry parameters not printed in the paper; context, not a target"}),
-          flush=True)
 
 
 def main():
@@ -404,11 +455,10 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="gsm", choices=["gsm", "reference"])
-    ap.add_argument("--table1", action="store_true", help="context: single-solve times on the paper's Table 1 shapes")
+    ap.add_argument("--flags", type=int, default=0, help="diagnostic plan flags (include/gsm.h GSM_FLAG_*), for A/B runs")
+    ap.add_argument("--levels", type=int, default=LEVELS, help="gsm_scan_mesh waves (1 = plain lock-step gsm_scan)")
     args = ap.parse_args()
-    if args.table1:
-        run_table1(args)
-    elif args.impl == "reference":
+    if args.impl == "reference":
         run_reference(args)
     else:
         run_gsm(args)

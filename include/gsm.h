@@ -56,6 +56,16 @@ enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2 };
  *       voxel path: transform of 1 - eps_b/eps_j.  gsm_plan_coeffs returns D_d.  `pol` is the amplitude h of H^inc. */
 enum { GSM_FORM_E = 0, GSM_FORM_H = 1 };
 
+/* Diagnostic flags of a plan (gsm_plan_desc.flags, 0 in normal use).  They select the general-purpose code path where
+ * a specialised one would be taken, so that tests can hold both to the same parity bar:
+ *   GSM_FLAG_TWO_SWEEP     Gram-Schmidt by the two-sweep kernels even where one field vector fits a thread-block cluster
+ *   GSM_FLAG_GENERIC_APPLY generic radix-2/4/8 FFT passes even where a 64- or 128-point fast path applies
+ *   GSM_FLAG_FUSED_APPLY   64-point fast path as ONE persistent launch that keeps the z-transformed intermediate in L2
+ *                          (apply_fused64.cu) instead of three launches through HBM; measured slower */
+enum { GSM_FLAG_TWO_SWEEP = 1, GSM_FLAG_GENERIC_APPLY = 2, GSM_FLAG_FUSED_APPLY = 4 };
+
+#define GSM_MAX_ITERS 512   /* largest accepted gsm_plan_desc.max_iters */
+
 /* One analytic inclusion ("Fourier images of sphere and polyhedron can be combined").
  * size = (R, -, -) for a sphere, semi-axes for an ellipsoid, full edge lengths for an axis-aligned box; same
  * length unit as the periods.  The inclusion's permittivity replaces the background inside it; overlapping
@@ -80,10 +90,11 @@ typedef struct {
     const gsm_shape* shapes;
     int voxels[3];
     const double* eps_grid_host;
-    int max_iters;               /* GMRES basis size (unrestarted); default 64 if <= 0                         */
+    int max_iters;               /* GMRES basis size (unrestarted); default 64 if <= 0; at most GSM_MAX_ITERS  */
     int max_batch;               /* (k, omega) points solved concurrently; default 1 if <= 0                   */
     void* cuda_stream;           /* cudaStream_t to enqueue on; NULL = the legacy default stream               */
     int formulation;             /* GSM_FORM_E (0) or GSM_FORM_H (1)                                           */
+    int flags;                   /* GSM_FLAG_* diagnostics, 0 in normal use                                    */
 } gsm_plan_desc;
 
 /* Build the plan on the current CUDA device: evaluate c_d (analytic closed forms or FFT of the voxel grid),
@@ -134,6 +145,23 @@ gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double k0, const d
 gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
                     double tol, double* resp_host, int* iters, double* resid, void* d_E_out);
 
+/* gsm_scan with an initial guess per point (Saad's GMRES with x0 != 0: r0 = b - A x0, solve A d = r0, E = x0 + d; the
+ * stop test stays relative to ||b||).  d_x0: device, [npts][3][N1][N2][N3] complex, or NULL (= gsm_scan); it may be the
+ * same buffer as d_E_out.  A guess whose residual is not below ||b|| is ignored for that point (zero start).  The
+ * reported iteration count excludes the one extra operator apply that forms r0. */
+gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                          double tol, const void* d_x0, double* resp_host, int* iters, double* resid, void* d_E_out);
+
+/* Scan of an ORDERED mesh: the list is a line in (k, omega) space sampled at equidistant parameter values in list order
+ * ("equidistant mesh kappa_p").  The points are solved in `levels` waves, coarse to fine: wave 0 takes
+ * every 2^(levels-1)-th point from a zero start, each later wave the points mid-way between those already solved,
+ * started from the Lagrange interpolation (up to 4 neighbours) of their solutions (gsm_scan_guess).  Where the
+ * responses solved so far show poles inside the mesh (the pole search of Eq. 7-10 in units of the list index), the
+ * interpolation is done on the field times prod (t - eta_k), which is smooth across a pole.  Same results as gsm_scan
+ * up to the solver tolerance, fewer iterations.  levels = 1 is gsm_scan.  Outputs as gsm_scan, in list order. */
+gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                         double tol, int levels, double* resp_host, int* iters, double* resid, void* d_E_out);
+
 /* Pole search, host side (Eq. 7-10, with xi in the numerator of Eq. 9 - DESIGN.md reading R11).
  * kappa[npts] equidistant and increasing, xi[npts] complex, npts >= Np + Nd.  All npts - Nd sliding windows of
  * Nd + 1 points are used (least squares).  eta[Np], zeta[Np] complex.  *best = index of the root with
@@ -147,12 +175,24 @@ gsm_status gsm_pole_search(int npts, const double* kappa, const double* xi, int 
  *      (3 complex), response = component `comp` of the 0-th order field; pole search (Np = 5, Nd = 10) -> estimate eta_c;
  *   2. fine scan: nfine points with spacing fine_step * k0 centred so that eta_c falls mid-way between the two middle
  *      nodes (a sample too close to the pole spoils the fit); pole search -> eta.
+ * comp = -1: response = projection of the 0-th order field on the amplitude (see gsm_retrieve_neff_many).
  * ncoarse, nfine >= 15 (= Np + Nd); nfine even.  out[0..1] = n_eff (re, im), out[2..3] = eps_eff = n_eff^2,
  * out[4..5] = pole amplitude zeta.  GSM_NOT_CONVERGED (warning) if a solve hit max_iters; GSM_E_INVALID if no pole with
  * Re eta inside the scanned window was found in either stage. */
 gsm_status gsm_retrieve_neff(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
                              double n_lo, double n_hi, int ncoarse, int nfine, double fine_step, double tol,
                              double out[6]);
+
+/* The same retrieval for many lines at once - the three (direction, polarisation) pairs of a tensor, a
+ * sweep over propagation directions at fixed omega (Fresnel normal surface), a frequency list
+ * (k0 differs per line) - with ALL lines' points of a stage in ONE gsm_scan, so that the lock-step batch stays full.
+ * dir[nlines][3] unit vectors, pol[nlines][6], comp[nlines] in {0, 1, 2} or -1 = projection of the 0-th order field on the
+ * amplitude (sum_c conj(a_c) E_c / |a|^2, for off-axis directions), k0, n_lo, n_hi [nlines].  out[nlines][6] as
+ * gsm_retrieve_neff (NaN for a line without a pole in its window); line_status[nlines] (may be NULL) GSM_OK or
+ * GSM_E_INVALID per line.  Returns GSM_E_INVALID if any line failed, after filling the others. */
+gsm_status gsm_retrieve_neff_many(gsm_plan* plan, int nlines, const double* dir, const double* pol, const int* comp,
+                                  const double* k0, const double* n_lo, const double* n_hi, int ncoarse, int nfine,
+                                  double fine_step, double tol, double* out, int* line_status);
 
 /* Text of the last failure on this plan (or of the last failed gsm_plan_create when plan == NULL). */
 const char* gsm_last_error(const gsm_plan* plan);

@@ -267,18 +267,31 @@ def solve_dense(c, periods, orders, k_inc, k0, eps_b, pol) -> np.ndarray:
 # --------------------------------------------------------------------------------------------------
 # a6-a8: full GMRES, modified Gram-Schmidt, Givens least squares       PAPER.md:105 (Saad [27], Alg. 6.9)
 # --------------------------------------------------------------------------------------------------
-def gmres(apply, b: np.ndarray, tol: float, max_iters: int):
-    """Unrestarted GMRES from x0 = 0 (reading R9).  <u,v> = sum conj(u) v.
+def gmres(apply, b: np.ndarray, tol: float, max_iters: int, x0: np.ndarray | None = None):
+    """Unrestarted GMRES (reading R9).  <u,v> = sum conj(u) v.
+
+    x0 = None: start from zero.  x0 given (the solution at the neighbouring kappa point of the
+    equidistant mesh): textbook form - r0 = b - A x0, GMRES on A d = r0, x = x0 + d (Saad Alg. 6.9
+    with a non-zero initial guess).  The stop test stays relative to ||b||, so every start meets the same bar.
 
     Returns (x, history, iters): history[j] = |g_{j+1}| / ||b|| after iteration j+1.
     Lucky breakdown (h_{j+1,j} = 0) exits as converged (reading R23).
     """
     shape = b.shape
     bv = b.ravel()
-    beta = np.linalg.norm(bv)
-    if beta == 0.0:
+    bnorm = np.linalg.norm(bv)
+    if bnorm == 0.0:
         return np.zeros(shape, np.complex128), [], 0
-    V = [bv / beta]
+    if x0 is None:
+        xs = np.zeros_like(bv)
+        r0 = bv
+    else:
+        xs = np.asarray(x0, dtype=np.complex128).ravel().copy()
+        r0 = bv - apply(xs.reshape(shape)).ravel()
+    beta = np.linalg.norm(r0)
+    if beta <= tol * bnorm:
+        return xs.reshape(shape), [], 0
+    V = [r0 / beta]
     H = np.zeros((max_iters + 1, max_iters), dtype=np.complex128)
     cs = np.zeros(max_iters)
     sn = np.zeros(max_iters, dtype=np.complex128)
@@ -311,24 +324,24 @@ def gmres(apply, b: np.ndarray, tol: float, max_iters: int):
         g[j + 1] = -np.conj(sn[j]) * g[j]
         g[j] = cs[j] * g[j]
         m = j + 1
-        hist.append(abs(g[j + 1]) / beta)
+        hist.append(abs(g[j + 1]) / bnorm)
         if hist[-1] <= tol or hn <= np.finfo(float).eps * beta:
             break
         V.append(w / hn)
     y = np.zeros(m, dtype=np.complex128)
     for i in range(m - 1, -1, -1):                               # back substitution
         y[i] = (g[i] - H[i, i + 1 : m] @ y[i + 1 : m]) / H[i, i]
-    x = np.zeros_like(bv)
+    x = xs.copy()
     for i in range(m):
         x += y[i] * V[i]
     return x.reshape(shape), hist, m
 
 
-def solve_gmres(c, periods, orders, k_inc, k0, eps_b, pol, tol=1e-13, max_iters=200, matvec=None):
+def solve_gmres(c, periods, orders, k_inc, k0, eps_b, pol, tol=1e-13, max_iters=200, matvec=None, x0=None):
     """Solve Eq. 4 by full GMRES with the O(n^2) Toeplitz product.  Returns (E, history, iters)."""
     mv = matvec or toeplitz_matvec
     b = incident(orders, pol)
-    return gmres(lambda v: apply_operator(c, v, periods, k_inc, k0, eps_b, mv), b, tol, max_iters)
+    return gmres(lambda v: apply_operator(c, v, periods, k_inc, k0, eps_b, mv), b, tol, max_iters, x0)
 
 
 # --------------------------------------------------------------------------------------------------

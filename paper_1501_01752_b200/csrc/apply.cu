@@ -195,36 +195,45 @@ size_t apply_smem_max(const ApplyGeom& g) {
     return m;
 }
 
-cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
-                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact) {
-    const int nlt = (g.NL + g.L - 1) / g.L;
-    // The batch can go through the three passes `sub` solves at a time through the SAME workspace W (stream order
-    // keeps sub-batches apart), which keeps W in L2; measured slower than one pass at 31^3 (see gsm_api.cu), so
-    // sub == batch unless GSM_APPLY_SUB is set.
-    const int sub = g.sub > 0 ? g.sub : batch;
-    const double Cb = 16.0 * g.ax[0].P * g.ax[1].P * g.ax[2].P;
-    for (int b0 = 0; b0 < batch; b0 += sub) {
-        const int nb = batch - b0 < sub ? batch - b0 : sub;
-        const double frac = (double)nact * nb / batch;
-        // algorithmic bytes of the three passes as designed: field vector V = 3n, z-transformed intermediate 3 P3 NL
-        const double V = 16.0 * 3.0 * g.n * frac, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL * frac;
-        const cplx* x = d_x + (long)b0 * 3 * g.n;
-        cplx* y = d_y + (long)b0 * 3 * g.n;
-        const double* kv = d_kvec + 3 * b0;
-        const double* k0 = d_k0 + b0;
-        const int* act = d_active ? d_active + b0 : nullptr;
-        { ProfScope ps_(prof, KC_Z_FORWARD, st, V + Wb);
-          if (g.chat64) launch_z_forward64(g, nb, x, d_W, kv, act, st);
-          else z_forward_kernel<<<dim3(nlt, 3, nb), 256, smem_pass1(g), st>>>(g, x, d_W, kv, act); }
-        { ProfScope ps_(prof, KC_XY_CONV, st, 2.0 * Wb + Cb);
-          if (g.chat64) launch_xy_conv64(g, nb, d_W, g.chat64, act, st);
-          else if (g.chat128) launch_xy_conv128(g, nb, d_W, g.chat128, act, st);
-          else xy_conv_kernel<<<dim3(g.ax[2].P, 3, nb), 256, smem_pass2(g), st>>>(g, d_W, act); }
-        { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st, Wb + 2.0 * V);
-          if (g.chat64) launch_z_inverse_green64(g, nb, d_W, x, y, kv, k0, act, st);
-          else z_inverse_green_kernel<<<dim3(nlt, nb), 256, smem_pass3(g), st>>>(g, d_W, x, y, kv, k0, act); }
+// algorithmic bytes of one solve-apply as designed: field vector V = 3n, z-transformed intermediate W_b = 3 P3 NL.
+// three launches: z_forward V + W_b, xy_conv 2 W_b, z_inverse_green W_b + 2 V; fused persistent launch: 2 V (W stays in L2).
+void bill_apply(const ApplyGeom& g, bool fused, Profiler* prof, double units) {
+    if (!prof || units <= 0.0) return;
+    const double V = 16.0 * 3.0 * g.n, Wb = 16.0 * 3.0 * g.ax[2].P * g.NL;
+    if (fused) {
+        prof->bytes[KC_APPLY_FUSED] += 2.0 * V * units;
+    } else {
+        prof->bytes[KC_Z_FORWARD] += (V + Wb) * units;
+        prof->bytes[KC_XY_CONV] += 2.0 * Wb * units;
+        prof->bytes[KC_Z_INVERSE_GREEN] += (Wb + 2.0 * V) * units;
     }
-    return cudaGetLastError();
+}
+
+cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
+                         cplx* d_y, cplx* d_W, const Fused64Dev* fused, const int* d_active, cudaStream_t st,
+                         Profiler* prof, double units) {
+    const double Cb = 16.0 * g.ax[0].P * g.ax[1].P * g.ax[2].P;   // the coefficient spectrum is read once per launch
+    cudaError_t e = cudaSuccess;
+    if (fused && fused->ring) {
+        bill_apply(g, true, prof, units);
+        ProfScope ps_(prof, KC_APPLY_FUSED, st, Cb);
+        return launch_apply_fused64(g, batch, d_kvec, d_k0, d_x, d_y, d_active, *fused, st);
+    }
+    bill_apply(g, false, prof, units);
+    const int nlt = (g.NL + g.L - 1) / g.L;
+    { ProfScope ps_(prof, KC_Z_FORWARD, st);
+      if (g.chat64) e = launch_z_forward64(g, batch, d_x, d_W, d_kvec, d_active, st);
+      else { z_forward_kernel<<<dim3(nlt, 3, batch), 256, smem_pass1(g), st>>>(g, d_x, d_W, d_kvec, d_active); e = cudaGetLastError(); } }
+    if (e != cudaSuccess) return e;
+    { ProfScope ps_(prof, KC_XY_CONV, st, Cb);
+      if (g.chat64) e = launch_xy_conv64(g, batch, d_W, g.chat64, d_active, st);
+      else if (g.chat128) e = launch_xy_conv128(g, batch, d_W, g.chat128, d_active, st);
+      else { xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); e = cudaGetLastError(); } }
+    if (e != cudaSuccess) return e;
+    { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st);
+      if (g.chat64) e = launch_z_inverse_green64(g, batch, d_W, d_x, d_y, d_kvec, d_k0, d_active, st);
+      else { z_inverse_green_kernel<<<dim3(nlt, batch), 256, smem_pass3(g), st>>>(g, d_W, d_x, d_y, d_kvec, d_k0, d_active); e = cudaGetLastError(); } }
+    return e;
 }
 
 }  // namespace gsm

@@ -277,8 +277,8 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
 }
 
 cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
-                                   int nclusters, cudaStream_t st, Profiler* prof, int nact) {
-    ProfScope ps_(prof, KC_ARNOLDI_MGS, st, 16.0 * d.vlen * (j + 3.0) * nact);   // reads w, v_0..v_j; writes v_{j+1}
+                                   int nclusters, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_ARNOLDI_MGS, st);   // (j + 3) V per solve still iterating, billed by run_batch afterwards
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(batch < nclusters ? batch : nclusters) * cs);
     cfg.blockDim = dim3(MGS_T);

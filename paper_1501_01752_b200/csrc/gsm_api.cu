@@ -21,6 +21,7 @@ struct gsm_plan {
     int max_batch = 1, max_iters = 64;
     long i0 = 0;                  // flat index of m = 0 inside one component
     int mgs_cs = 0, mgs_chunk = 0, mgs_nclusters = 0; // cluster MGS Arnoldi step (0 = two-sweep fallback)
+    Fused64Dev fused;             // fused persistent apply for 64-point axes (ring == null: three-launch apply)
     std::vector<void*> allocs;    // every device allocation, freed in destroy
     long long device_bytes = 0;
     Profiler prof;
@@ -35,6 +36,10 @@ struct gsm_plan {
     int* vpos[3] = {nullptr, nullptr, nullptr};
     int vdim[3] = {0, 0, 0};
     double *d_kvec = nullptr, *d_k0 = nullptr, *d_resid = nullptr;
+    cplx* mesh_fields = nullptr;  // gsm_scan_mesh without d_E_out: every solution of the mesh (grown on demand)
+    size_t mesh_cap = 0;
+    int *d_mesh_idx = nullptr, *d_mesh_nbr = nullptr;   // [max_batch], [max_batch][4]
+    cplx* d_mesh_wgt = nullptr;                         // [max_batch][4]
     void* pinned = nullptr;       // host staging: nactive, iters, resid, hist
     size_t pinned_bytes = 0;
     mutable std::string err;
@@ -220,12 +225,13 @@ static gsm_status build_spectrum(gsm_plan* plan) {
     if (e == cudaSuccess) e = launch_fft_axis(pad, (long)P[0], full[1], P[2], g.tw[1], plan->stream);
     if (e == cudaSuccess) e = launch_fft_axis(pad, 1, full[0], (long)P[1] * P[2], g.tw[0], plan->stream);
     if (e == cudaSuccess) e = launch_chat_layout(pad, P, plan->chat, plan->stream);
-    if (e == cudaSuccess && apply64_usable(g) && !getenv("GSM_GENERIC_APPLY")) {
+    const bool generic = (plan->desc.flags & GSM_FLAG_GENERIC_APPLY) != 0;
+    if (e == cudaSuccess && apply64_usable(g) && !generic) {
         if (!plan->chat64) CK(dalloc(plan, &plan->chat64, np));
         e = launch_chat64_layout(plan->chat, plan->chat64, plan->stream);
         g.chat64 = plan->chat64;
     }
-    if (e == cudaSuccess && apply128_usable(g) && !getenv("GSM_GENERIC_APPLY")) {
+    if (e == cudaSuccess && apply128_usable(g) && !generic) {
         if (!plan->chat128) {
             CK(dalloc(plan, &plan->chat128, np));
             for (int a = 0; a < 2; ++a) {   // new position -> frequency -> position in the generic network
@@ -253,6 +259,10 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
     if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(nullptr, GSM_E_INVALID, "eps_b must be non-zero");
     if (desc->eps_grid_host == nullptr && (desc->n_shapes < 0 || (desc->n_shapes > 0 && !desc->shapes)))
         return fail(nullptr, GSM_E_INVALID, "shapes missing");
+    // the two-sweep kernels stage (j + 1)-sized rows in shared memory and the pool holds max_iters + 1 vectors per solve
+    if (desc->max_iters > GSM_MAX_ITERS) return fail(nullptr, GSM_E_INVALID, "max_iters exceeds GSM_MAX_ITERS");
+    if (desc->flags & ~(GSM_FLAG_TWO_SWEEP | GSM_FLAG_GENERIC_APPLY | GSM_FLAG_FUSED_APPLY))
+        return fail(nullptr, GSM_E_INVALID, "unknown flag");
     gsm_plan* plan = new (std::nothrow) gsm_plan();
     if (!plan) return fail(nullptr, GSM_E_ALLOC, "host allocation failed");
     plan->desc = *desc;
@@ -302,14 +312,27 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         kd.ld = m + 1;
         KrylovState& ks = plan->ks;
         CK(arnoldi_cluster_plan(kd, &plan->mgs_cs, &plan->mgs_chunk, &plan->mgs_nclusters));
-        if (getenv("GSM_FORCE_TWO_SWEEP")) plan->mgs_cs = 0;
-        {   // Sub-batching the apply so that W stays in L2 was measured and LOSES at 31^3 (sub = 8/16/32: step 208/185/
-            // 173 ms vs 157 ms for the whole batch: short kernels pay launch gaps and tails), so the default is one pass.
-            int sub = B;
-            if (const char* e = getenv("GSM_APPLY_SUB")) sub = atoi(e);
-            g.sub = std::max(1, std::min(B, sub));
+        if (desc->flags & GSM_FLAG_TWO_SWEEP) plan->mgs_cs = 0;
+        if (g.chat64 && (desc->flags & GSM_FLAG_FUSED_APPLY)) {
+            // fused persistent apply: W lives in a ring of a few solve slots that stays in L2 (apply_fused64.cu)
+            Fused64Dev& f = plan->fused;
+            CK(apply_fused64_init_attributes(&f.grid));
+            f.maxB = B;
+            int* items = nullptr;
+            const int ips = fused64_items_per_slot(g);
+            std::vector<int> pattern(ips);
+            fused64_slot_pattern(g, pattern.data());
+            CK(dalloc(plan, &items, (size_t)ips));
+            CK(cudaMemcpy(items, pattern.data(), sizeof(int) * ips, cudaMemcpyHostToDevice));
+            f.items = items;
+            CK(dalloc(plan, &f.head, (size_t)1));
+            CK(dalloc(plan, &f.nact, (size_t)1));
+            CK(dalloc(plan, &f.cnt, (size_t)3 * B));
+            CK(dalloc(plan, &f.list, (size_t)B));
+            CK(dalloc(plan, &f.ring, fused64_ring_elems(g)));
+        } else {
+            CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
         }
-        CK(dalloc(plan, &plan->W, (size_t)g.sub * 3 * g.ax[2].P * g.NL));
         CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &plan->ybuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &ks.basis, (size_t)kd.ld * B * kd.vlen));
@@ -323,6 +346,11 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &ks.ycoef, (size_t)B * kd.mmax));
         CK(dalloc(plan, &ks.hist, (size_t)B * kd.mmax));
         CK(dalloc(plan, &ks.beta, (size_t)B));
+        CK(dalloc(plan, &ks.bnorm, (size_t)B));
+        CK(dalloc(plan, &ks.guess, (size_t)B));
+        CK(dalloc(plan, &plan->d_mesh_idx, (size_t)B));
+        CK(dalloc(plan, &plan->d_mesh_nbr, (size_t)4 * B));
+        CK(dalloc(plan, &plan->d_mesh_wgt, (size_t)4 * B));
         CK(dalloc(plan, &ks.scale, (size_t)B));
         CK(dalloc(plan, &ks.active, (size_t)B));
         CK(dalloc(plan, &ks.iters, (size_t)B));
@@ -354,6 +382,7 @@ extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
     plan->prof.destroy();
     for (cudaEvent_t e : plan->iter_ev) if (e) cudaEventDestroy(e);
     for (void* p : plan->allocs) cudaFree(p);
+    if (plan->mesh_fields) cudaFree(plan->mesh_fields);
     if (plan->pinned) cudaFreeHost(plan->pinned);
     delete plan;
     return GSM_OK;
@@ -421,14 +450,15 @@ extern "C" gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch
     CK(cudaMemcpyAsync(plan->d_kvec, k_bloch, sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, plan->stream));
     CK(cudaMemcpyAsync(plan->d_k0, k0, sizeof(double) * batch, cudaMemcpyHostToDevice, plan->stream));
     CK(launch_apply(plan->geom, batch, plan->d_kvec, plan->d_k0, static_cast<const cplx*>(d_x), static_cast<cplx*>(d_y),
-                    plan->W, nullptr, plan->stream, &plan->prof, batch));
+                    plan->W, &plan->fused, nullptr, plan->stream, &plan->prof, (double)batch));
     return GSM_OK;
 }
 
-// nb <= max_batch solves in lock step.  d_E: device [nb][vlen].  Host outputs may be null.
+// nb <= max_batch solves in lock step.  d_E: device [nb][vlen].  d_x0 (may be null, may alias d_E): initial guesses.
+// Host outputs may be null.
 static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const double* k0, const double* pol, double tol,
-                            cplx* d_E, double* resp, int* iters, double* resid, double* hist, int hist_cap,
-                            bool* not_converged) {
+                            const cplx* d_x0, cplx* d_E, double* resp, int* iters, double* resid, double* hist,
+                            int hist_cap, bool* not_converged) {
     const KrylovDims& kd = plan->kd;
     const KrylovState& ks = plan->ks;
     const ApplyGeom& g = plan->geom;
@@ -445,18 +475,25 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     Profiler* prof = &plan->prof;
     CK(launch_krylov_init(kd, ks, nb, plan->i0, g.n, st, prof));
     const size_t vs = (size_t)nb * kd.vlen;
-    int j = 0, nact = nb;   // nact: solves still iterating (read back once per iteration)
+    if (d_x0) {   // r0 = b - A x0 (one more apply), v_0 = r0 / ||r0||; GMRES then solves A d = r0 and E = x0 + d
+        CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_x0, ks.basis + vs, plan->W, &plan->fused, nullptr, st, prof,
+                        (double)nb));
+        CK(launch_krylov_guess(kd, ks, nb, plan->i0, g.n, st, prof));
+    }
+    // Launches of the iteration loop are billed (algorithmic bytes) after the batch, from the final iteration counts:
+    // the host learns how many solves were still iterating one iteration late.
+    int j = 0;
     for (; j < kd.mmax; ++j) {
         CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
-                        plan->W, ks.active, st, prof, nact));
+                        plan->W, &plan->fused, ks.active, st, prof, 0.0));
         if (plan->mgs_cs > 0) {
-            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, st, prof, nact));
+            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, st, prof));
         } else {
-            CK(launch_sweep_dots(kd, ks, nb, j, st, prof, nact));
+            CK(launch_sweep_dots(kd, ks, nb, j, st, prof));
             CK(launch_hsolve(kd, ks, nb, j, st, prof));
-            CK(launch_sweep_update(kd, ks, nb, j, st, prof, nact));
+            CK(launch_sweep_update(kd, ks, nb, j, st, prof));
             CK(launch_givens(kd, ks, nb, j, st, prof));
-            CK(launch_normalize(kd, ks, nb, j, st, prof, nact));
+            CK(launch_normalize(kd, ks, nb, j, st, prof));
         }
         // The count of solves still iterating comes back one iteration late: iteration j + 1 is enqueued before the
         // host looks at the count after iteration j - 1, so launches never wait for a round trip.  If everything had
@@ -465,14 +502,13 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
         CK(cudaEventRecord(plan->iter_ev[j & 1], st));
         if (j >= 1) {
             CK(cudaEventSynchronize(plan->iter_ev[(j - 1) & 1]));
-            nact = pin_i[(j - 1) & 1];
-            if (nact <= 0) break;
+            if (pin_i[(j - 1) & 1] <= 0) break;
         }
     }
     CK(launch_backsolve(kd, ks, nb, st, prof));
-    CK(launch_combine(kd, ks, nb, d_E, st, prof));
+    CK(launch_combine(kd, ks, nb, d_x0, d_E, st, prof));
     // true residual with one more apply
-    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, nullptr, st, prof, nb));
+    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, &plan->fused, nullptr, st, prof, (double)nb));
     CK(launch_true_residual(kd, ks, nb, plan->ybuf, plan->i0, g.n, plan->d_resid, st, prof));
     int* h_iters = reinterpret_cast<int*>(pin + 2);
     double* h_resid = pin + 2 + nb;           // ints occupy at most nb doubles
@@ -488,6 +524,20 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
         CK(cudaMemcpyAsync(pin + 2 + 9 * (size_t)nb, ks.hist, sizeof(double) * std::min(hist_cap, kd.mmax),
                            cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    {   // bill the iteration loop: solve b ran iterations j = 0 .. m_b - 1, each one apply and one Arnoldi step
+        double s1 = 0.0, s2 = 0.0;   // sum m_b, sum m_b (m_b - 1) / 2
+        for (int b = 0; b < nb; ++b) { const double m = h_iters[b]; s1 += m; s2 += 0.5 * m * (m - 1.0); }
+        const double V = 16.0 * kd.vlen;
+        bill_apply(g, plan->fused.ring != nullptr, prof, s1);
+        if (plan->mgs_cs > 0) {
+            prof->bytes[KC_ARNOLDI_MGS] += V * (s2 + 3.0 * s1);       // (j + 3) V: w, v_0..v_j, write v_{j+1}
+        } else {
+            prof->bytes[KC_SWEEP_DOTS] += V * (s2 + 2.0 * s1);        // (j + 2) V
+            prof->bytes[KC_SWEEP_UPDATE] += V * (s2 + 3.0 * s1);      // (j + 3) V
+            prof->bytes[KC_NORMALIZE] += V * 2.0 * s1;
+        }
+        prof->bytes[KC_COMBINE] += V * (s1 + nb);                     // x = sum y_i v_i: m_b reads, one write
+    }
     for (int b = 0; b < nb; ++b) {
         if (iters) iters[b] = h_iters[b];
         if (resid) resid[b] = h_resid[b];
@@ -507,24 +557,170 @@ extern "C" gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double 
     if (!plan) return GSM_E_INVALID;
     if (!k_bloch || !pol || !d_E_out || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_solve: bad argument");
     bool nc = false;
-    gsm_status s = run_batch(plan, 1, k_bloch, &k0, pol, tol, static_cast<cplx*>(d_E_out), nullptr, n_iters,
+    gsm_status s = run_batch(plan, 1, k_bloch, &k0, pol, tol, nullptr, static_cast<cplx*>(d_E_out), nullptr, n_iters,
                              true_rel_resid, resid_hist_host, hist_cap, &nc);
     if (s != GSM_OK) return s;
     return nc ? GSM_NOT_CONVERGED : GSM_OK;
 }
 
-extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
-                               double tol, double* resp_host, int* iters, double* resid, void* d_E_out) {
+extern "C" gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                                     double tol, const void* d_x0, double* resp_host, int* iters, double* resid,
+                                     void* d_E_out) {
     if (!plan) return GSM_E_INVALID;
     if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_scan: bad argument");
     bool nc = false;
     for (int p0 = 0; p0 < npts; p0 += plan->max_batch) {
         const int nb = std::min(plan->max_batch, npts - p0);
         cplx* dE = d_E_out ? static_cast<cplx*>(d_E_out) + (size_t)p0 * plan->kd.vlen : plan->xbuf;
-        gsm_status s = run_batch(plan, nb, k_bloch + 3 * (size_t)p0, k0 + p0, pol + 6 * (size_t)p0, tol, dE,
+        const cplx* x0 = d_x0 ? static_cast<const cplx*>(d_x0) + (size_t)p0 * plan->kd.vlen : nullptr;
+        gsm_status s = run_batch(plan, nb, k_bloch + 3 * (size_t)p0, k0 + p0, pol + 6 * (size_t)p0, tol, x0, dE,
                                  resp_host ? resp_host + 6 * (size_t)p0 : nullptr, iters ? iters + p0 : nullptr,
                                  resid ? resid + p0 : nullptr, nullptr, 0, &nc);
         if (s != GSM_OK) return s;
+    }
+    return nc ? GSM_NOT_CONVERGED : GSM_OK;
+}
+
+extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                               double tol, double* resp_host, int* iters, double* resid, void* d_E_out) {
+    return gsm_scan_guess(plan, npts, k_bloch, k0, pol, tol, nullptr, resp_host, iters, resid, d_E_out);
+}
+
+// Lagrange weights at position t of the interpolation nodes tn[0..cnt)
+static void lagrange_weights(double t, const int* tn, int cnt, double* w) {
+    for (int a = 0; a < cnt; ++a) {
+        double v = 1.0;
+        for (int b = 0; b < cnt; ++b)
+            if (b != a) v *= (t - tn[b]) / (double)(tn[a] - tn[b]);
+        w[a] = v;
+    }
+}
+
+extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
+                                    double tol, int levels, double* resp_host, int* iters, double* resid, void* d_E_out) {
+    if (!plan) return GSM_E_INVALID;
+    if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0) || levels < 1 || levels > 16)
+        return fail(plan, GSM_E_INVALID, "gsm_scan_mesh: bad argument");
+    if (npts == 0) return GSM_OK;
+    while (levels > 1 && (1 << (levels - 1)) >= npts) --levels;
+    const size_t vlen = (size_t)plan->kd.vlen;
+    cplx* all = static_cast<cplx*>(d_E_out);
+    if (!all) {
+        if (plan->mesh_cap < (size_t)npts) {
+            if (plan->mesh_fields) cudaFree(plan->mesh_fields);
+            plan->mesh_fields = nullptr;
+            plan->mesh_cap = 0;
+            CK(cudaMalloc(reinterpret_cast<void**>(&plan->mesh_fields), sizeof(cplx) * vlen * npts));
+            plan->mesh_cap = (size_t)npts;
+        }
+        all = plan->mesh_fields;
+    }
+    const int B = plan->max_batch;
+    std::vector<double> kb(3 * (size_t)B), kk(B), pl(6 * (size_t)B), wgt(8 * (size_t)B), h_resp(6 * (size_t)B), h_resid(B);
+    std::vector<int> idx(B), nbr(4 * (size_t)B), h_iters(B);
+    std::vector<double> xi_all(2 * (size_t)npts, 0.0);   // response projected on the amplitude, for the pole estimate
+    bool nc = false;
+    const int s0 = 1 << (levels - 1);
+    for (int lev = 0; lev < levels; ++lev) {
+        // wave 0: multiples of s0 from x0 = 0; wave lev: odd multiples of sl = s0 >> lev, whose neighbours at distance
+        // sl and 3 sl are multiples of 2 sl, i.e. solved by an earlier wave
+        const int sl = s0 >> lev;
+        // Near a pole eta of the response the field behaves as R / (kappa - eta) + smooth, which
+        // polynomial interpolation follows badly - and those are the points that need most iterations.  The solved
+        // points (multiples of 2 sl: an equidistant mesh) give the poles in units of the list index through the
+        // pole search of Eq. 7-10; the guess then interpolates prod_k (t - eta_k) E(t), which is smooth, and divides
+        // the product out at the target.  Only the guess changes: the solves and their stop test do not.
+        const int Np = 5, Nd = 10;
+        double pe[2 * Np];
+        int npole = 0;
+        if (lev > 0 && (npts - 1) / (2 * sl) + 1 >= Np + Nd) {
+            const int cnt = (npts - 1) / (2 * sl) + 1;
+            std::vector<double> tt(cnt), xs(2 * (size_t)cnt);
+            for (int i = 0; i < cnt; ++i) {
+                tt[i] = (double)(2 * sl) * i;
+                xs[2 * i] = xi_all[2 * (size_t)(2 * sl * i)];
+                xs[2 * i + 1] = xi_all[2 * (size_t)(2 * sl * i) + 1];
+            }
+            double eta[2 * Np], zeta[2 * Np];
+            int best = -1;
+            if (gsm_pole_search(cnt, tt.data(), xs.data(), Np, Nd, tt.front(), tt.back(), eta, zeta, &best) == GSM_OK && best >= 0) {
+                const double zmax = std::hypot(zeta[2 * best], zeta[2 * best + 1]);
+                for (int k = 0; k < Np; ++k)      // every pole inside the mesh whose amplitude matters
+                    if (eta[2 * k] >= tt.front() && eta[2 * k] <= tt.back() &&
+                        std::hypot(zeta[2 * k], zeta[2 * k + 1]) >= 1e-6 * zmax) {
+                        pe[2 * npole] = eta[2 * k];
+                        pe[2 * npole + 1] = eta[2 * k + 1];
+                        ++npole;
+                    }
+            }
+        }
+        const int first = lev == 0 ? 0 : sl, step = lev == 0 ? s0 : 2 * sl;
+        for (int p0 = first; p0 < npts;) {
+            int nb = 0;
+            for (; nb < B && p0 < npts; ++nb, p0 += step) {
+                const int p = p0;
+                idx[nb] = p;
+                for (int a = 0; a < 3; ++a) kb[3 * nb + a] = k_bloch[3 * (size_t)p + a];
+                kk[nb] = k0[p];
+                for (int q = 0; q < 6; ++q) pl[6 * nb + q] = pol[6 * (size_t)p + q];
+                if (lev > 0) {
+                    int nodes[4], cnt = 0;
+                    const int cand[4] = {p - 3 * sl, p - sl, p + sl, p + 3 * sl};
+                    for (int q = 0; q < 4; ++q)
+                        if (cand[q] >= 0 && cand[q] < npts) nodes[cnt++] = cand[q];
+                    double w[4];
+                    lagrange_weights((double)p, nodes, cnt, w);
+                    for (int q = 0; q < 4; ++q) {
+                        nbr[4 * nb + q] = q < cnt ? nodes[q] : -1;
+                        double wr = q < cnt ? w[q] : 0.0, wi = 0.0;
+                        for (int k = 0; k < npole && q < cnt; ++k) {   // times (t_q - eta_k) / (t_p - eta_k)
+                            const double ar = nodes[q] - pe[2 * k], ai = -pe[2 * k + 1];
+                            const double br = p - pe[2 * k], bi = -pe[2 * k + 1];
+                            const double inv = 1.0 / (br * br + bi * bi);
+                            const double fr = (ar * br + ai * bi) * inv, fi = (ai * br - ar * bi) * inv;
+                            const double tr = wr * fr - wi * fi;
+                            wi = wr * fi + wi * fr;
+                            wr = tr;
+                        }
+                        if (!std::isfinite(wr) || !std::isfinite(wi)) { wr = q < cnt ? w[q] : 0.0; wi = 0.0; }
+                        wgt[8 * nb + 2 * q] = wr;
+                        wgt[8 * nb + 2 * q + 1] = wi;
+                    }
+                }
+            }
+            cudaStream_t st = plan->stream;
+            CK(cudaMemcpyAsync(plan->d_mesh_idx, idx.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
+            const cplx* x0 = nullptr;
+            if (lev > 0) {
+                CK(cudaMemcpyAsync(plan->d_mesh_nbr, nbr.data(), sizeof(int) * 4 * nb, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(plan->d_mesh_wgt, wgt.data(), sizeof(cplx) * 4 * nb, cudaMemcpyHostToDevice, st));
+                CK(launch_mesh_guess(plan->kd, nb, all, plan->d_mesh_nbr, plan->d_mesh_wgt, plan->xbuf, st, &plan->prof));
+                CK(cudaStreamSynchronize(st));   // the host vectors are rewritten by the next chunk
+                x0 = plan->xbuf;
+            }
+            gsm_status s = run_batch(plan, nb, kb.data(), kk.data(), pl.data(), tol, x0, plan->xbuf, h_resp.data(),
+                                     h_iters.data(), h_resid.data(), nullptr, 0, &nc);
+            if (s != GSM_OK) return s;
+            CK(launch_mesh_scatter(plan->kd, nb, plan->xbuf, plan->d_mesh_idx, all, st, &plan->prof));
+            CK(cudaStreamSynchronize(st));
+            for (int b = 0; b < nb; ++b) {
+                const size_t p = (size_t)idx[b];
+                if (resp_host) for (int q = 0; q < 6; ++q) resp_host[6 * p + q] = h_resp[6 * b + q];
+                {   // xi = sum_c conj(a_c) E_c / |a|^2
+                    const double* a = pol + 6 * p;
+                    double re = 0.0, im = 0.0, nrm = 0.0;
+                    for (int c = 0; c < 3; ++c) {
+                        re += a[2 * c] * h_resp[6 * b + 2 * c] + a[2 * c + 1] * h_resp[6 * b + 2 * c + 1];
+                        im += a[2 * c] * h_resp[6 * b + 2 * c + 1] - a[2 * c + 1] * h_resp[6 * b + 2 * c];
+                        nrm += a[2 * c] * a[2 * c] + a[2 * c + 1] * a[2 * c + 1];
+                    }
+                    xi_all[2 * p] = nrm > 0.0 ? re / nrm : 0.0;
+                    xi_all[2 * p + 1] = nrm > 0.0 ? im / nrm : 0.0;
+                }
+                if (iters) iters[p] = h_iters[b];
+                if (resid) resid[p] = h_resid[b];
+            }
+        }
     }
     return nc ? GSM_NOT_CONVERGED : GSM_OK;
 }
@@ -534,7 +730,7 @@ extern "C" gsm_status gsm_scan(gsm_plan* plan, int npts, const double* k_bloch, 
 namespace gsm {
 static const char* const kKernelClassNames[KC_COUNT] = {
     "z_forward", "xy_conv", "z_inverse_green", "sweep_dots", "hsolve", "sweep_update", "givens", "normalize",
-    "arnoldi_mgs", "combine", "residual", "small", "plan"};
+    "arnoldi_mgs", "combine", "residual", "small", "plan", "apply_fused"};
 const char* kernel_class_name(int cls) { return cls >= 0 && cls < KC_COUNT ? kKernelClassNames[cls] : ""; }
 
 void Profiler::begin(int c, cudaStream_t st, double nbytes) {
@@ -617,6 +813,18 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
     if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(plan, GSM_E_INVALID, "eps_b must be non-zero");
     if (desc->eps_grid_host == nullptr && (desc->n_shapes < 0 || (desc->n_shapes > 0 && !desc->shapes)))
         return fail(plan, GSM_E_INVALID, "shapes missing");
+    if (desc->formulation != plan->desc.formulation) return fail(plan, GSM_E_INVALID, "gsm_plan_set_cell: formulation differs");
+    if (desc->eps_grid_host) {
+        AxisPlan tmp;
+        for (int a = 0; a < 3; ++a)
+            if (desc->voxels[a] < 2 * desc->orders[a] - 1 || desc->voxels[a] > 512 || !make_axis(desc->voxels[a], desc->voxels[a], &tmp))
+                return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
+    } else {
+        for (int i = 0; i < desc->n_shapes; ++i)
+            if (desc->shapes[i].kind != GSM_SPHERE && desc->shapes[i].kind != GSM_ELLIPSOID && desc->shapes[i].kind != GSM_BOX)
+                return fail(plan, GSM_E_INVALID, "unknown shape kind");
+    }
+    // everything that can be rejected has been: from here on the plan's cell is replaced
     plan->desc.eps_bg_re = desc->eps_bg_re; plan->desc.eps_bg_im = desc->eps_bg_im;
     plan->desc.eps_b_re = desc->eps_b_re;   plan->desc.eps_b_im = desc->eps_b_im;
     plan->desc.n_shapes = desc->n_shapes;   plan->desc.shapes = desc->shapes;
@@ -640,49 +848,103 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
 
 
 // ---- retrieval (a10): two-stage scan + pole search -> n_eff, eps_eff -----------------------------------------------
-static gsm_status scan_line(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
-                            const std::vector<double>& kappa, double tol, std::vector<double>& xi, bool* warn) {
-    const int n = (int)kappa.size();
-    std::vector<double> kb(3 * (size_t)n), kk(n, k0), pl(6 * (size_t)n), resp(6 * (size_t)n);
-    for (int i = 0; i < n; ++i) {
-        for (int a = 0; a < 3; ++a) kb[3 * i + a] = kappa[i] * dir[a];
-        for (int q = 0; q < 6; ++q) pl[6 * i + q] = pol[q];
-    }
-    const gsm_status st = gsm_scan(plan, n, kb.data(), kk.data(), pl.data(), tol, resp.data(), nullptr, nullptr, nullptr);
+// One stage of the retrieval for many lines at once: line l scans kappa[l][0..n) along dir[l] with amplitude pol[l] at
+// k0[l]; ALL points go through ONE gsm_scan.  xi[l][i] = component comp[l] of the 0-th order field, or, for
+// comp[l] == -1, its projection on the amplitude, sum_c conj(a_c) E_c / sum_c |a_c|^2 (off-axis directions).
+static gsm_status scan_lines(gsm_plan* plan, int nl, const double* dir, const double* pol, const int* comp, const double* k0,
+                             const std::vector<double>& kappa, int n, double tol, std::vector<double>& xi, bool* warn) {
+    const size_t np = (size_t)nl * n;
+    std::vector<double> kb(3 * np), kk(np), pl(6 * np), resp(6 * np);
+    for (int l = 0; l < nl; ++l)
+        for (int i = 0; i < n; ++i) {
+            const size_t p = (size_t)l * n + i;
+            for (int a = 0; a < 3; ++a) kb[3 * p + a] = kappa[p] * dir[3 * l + a];
+            for (int q = 0; q < 6; ++q) pl[6 * p + q] = pol[6 * l + q];
+            kk[p] = k0[l];
+        }
+    const gsm_status st = gsm_scan(plan, (int)np, kb.data(), kk.data(), pl.data(), tol, resp.data(), nullptr, nullptr, nullptr);
     if (st < 0) return st;
     if (st == GSM_NOT_CONVERGED) *warn = true;
-    xi.resize(2 * (size_t)n);
-    for (int i = 0; i < n; ++i) { xi[2 * i] = resp[6 * i + 2 * comp]; xi[2 * i + 1] = resp[6 * i + 2 * comp + 1]; }
+    xi.resize(2 * np);
+    for (int l = 0; l < nl; ++l) {
+        const double* a = pol + 6 * l;
+        const double nrm = a[0] * a[0] + a[1] * a[1] + a[2] * a[2] + a[3] * a[3] + a[4] * a[4] + a[5] * a[5];
+        for (int i = 0; i < n; ++i) {
+            const size_t p = (size_t)l * n + i;
+            if (comp[l] >= 0) {
+                xi[2 * p] = resp[6 * p + 2 * comp[l]];
+                xi[2 * p + 1] = resp[6 * p + 2 * comp[l] + 1];
+            } else {
+                double re = 0.0, im = 0.0;
+                for (int c = 0; c < 3; ++c) {   // conj(a_c) E_c
+                    re += a[2 * c] * resp[6 * p + 2 * c] + a[2 * c + 1] * resp[6 * p + 2 * c + 1];
+                    im += a[2 * c] * resp[6 * p + 2 * c + 1] - a[2 * c + 1] * resp[6 * p + 2 * c];
+                }
+                xi[2 * p] = re / nrm;
+                xi[2 * p + 1] = im / nrm;
+            }
+        }
+    }
     return GSM_OK;
+}
+
+extern "C" gsm_status gsm_retrieve_neff_many(gsm_plan* plan, int nlines, const double* dir, const double* pol, const int* comp,
+                                             const double* k0, const double* n_lo, const double* n_hi, int ncoarse,
+                                             int nfine, double fine_step, double tol, double* out, int* line_status) {
+    if (!plan) return GSM_E_INVALID;
+    const int Np = 5, Nd = 10;
+    if (nlines < 0 || !dir || !pol || !comp || !k0 || !n_lo || !n_hi || !out || ncoarse < Np + Nd || nfine < Np + Nd ||
+        (nfine & 1) || !(fine_step > 0.0) || !(tol > 0.0))
+        return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: bad argument");
+    for (int l = 0; l < nlines; ++l)
+        if (comp[l] < -1 || comp[l] > 2 || !(k0[l] > 0.0) || !(n_hi[l] > n_lo[l]))
+            return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: bad argument");
+    if (nlines == 0) return GSM_OK;
+    bool warn = false, missing = false;
+    std::vector<double> kappa((size_t)nlines * ncoarse), xi, eta_c(nlines, 0.0);
+    std::vector<int> ok(nlines, 1);
+    for (int l = 0; l < nlines; ++l)
+        for (int i = 0; i < ncoarse; ++i)
+            kappa[(size_t)l * ncoarse + i] = k0[l] * (n_lo[l] + (n_hi[l] - n_lo[l]) * i / (ncoarse - 1));
+    gsm_status st = scan_lines(plan, nlines, dir, pol, comp, k0, kappa, ncoarse, tol, xi, &warn);
+    if (st < 0) return st;
+    double eta[2 * Np], zeta[2 * Np];
+    for (int l = 0; l < nlines; ++l) {
+        int best = -1;
+        const double* kp = kappa.data() + (size_t)l * ncoarse;
+        st = gsm_pole_search(ncoarse, kp, xi.data() + 2 * (size_t)l * ncoarse, Np, Nd, kp[0], kp[ncoarse - 1], eta, zeta, &best);
+        if (st < 0 || best < 0) { ok[l] = 0; missing = true; eta_c[l] = 0.5 * (kp[0] + kp[ncoarse - 1]); }
+        else eta_c[l] = eta[2 * best];
+    }
+    kappa.assign((size_t)nlines * nfine, 0.0);
+    for (int l = 0; l < nlines; ++l)
+        for (int i = 0; i < nfine; ++i)      // nfine even: the estimate falls mid-way between the two middle nodes
+            kappa[(size_t)l * nfine + i] = eta_c[l] + fine_step * k0[l] * (i - 0.5 * (nfine - 1));
+    st = scan_lines(plan, nlines, dir, pol, comp, k0, kappa, nfine, tol, xi, &warn);
+    if (st < 0) return st;
+    for (int l = 0; l < nlines; ++l) {
+        double* o = out + 6 * (size_t)l;
+        int best = -1;
+        const double* kp = kappa.data() + (size_t)l * nfine;
+        if (ok[l]) st = gsm_pole_search(nfine, kp, xi.data() + 2 * (size_t)l * nfine, Np, Nd, kp[0], kp[nfine - 1], eta, zeta, &best);
+        if (!ok[l] || st < 0 || best < 0) {
+            ok[l] = 0; missing = true;
+            for (int q = 0; q < 6; ++q) o[q] = NAN;
+        } else {
+            const double nr = eta[2 * best] / k0[l], ni = eta[2 * best + 1] / k0[l];
+            o[0] = nr; o[1] = ni;
+            o[2] = nr * nr - ni * ni; o[3] = 2.0 * nr * ni;
+            o[4] = zeta[2 * best]; o[5] = zeta[2 * best + 1];
+        }
+        if (line_status) line_status[l] = ok[l] ? GSM_OK : GSM_E_INVALID;
+    }
+    if (missing) return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: no pole inside the scanned window of at least one line");
+    return warn ? GSM_NOT_CONVERGED : GSM_OK;
 }
 
 extern "C" gsm_status gsm_retrieve_neff(gsm_plan* plan, const double dir[3], const double pol[6], int comp, double k0,
                                         double n_lo, double n_hi, int ncoarse, int nfine, double fine_step, double tol,
                                         double out[6]) {
-    if (!plan) return GSM_E_INVALID;
-    const int Np = 5, Nd = 10;
-    if (!dir || !pol || !out || comp < 0 || comp > 2 || !(k0 > 0.0) || !(n_hi > n_lo) || ncoarse < Np + Nd ||
-        nfine < Np + Nd || (nfine & 1) || !(fine_step > 0.0) || !(tol > 0.0))
-        return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: bad argument");
-    bool warn = false;
-    std::vector<double> kappa(ncoarse), xi;
-    for (int i = 0; i < ncoarse; ++i) kappa[i] = k0 * (n_lo + (n_hi - n_lo) * i / (ncoarse - 1));
-    gsm_status st = scan_line(plan, dir, pol, comp, k0, kappa, tol, xi, &warn);
-    if (st < 0) return st;
-    double eta[2 * Np], zeta[2 * Np];
-    int best = -1;
-    st = gsm_pole_search(ncoarse, kappa.data(), xi.data(), Np, Nd, kappa.front(), kappa.back(), eta, zeta, &best);
-    if (st < 0 || best < 0) return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: no pole inside the coarse window");
-    const double eta_c = eta[2 * best], h = fine_step * k0;
-    kappa.resize(nfine);
-    for (int i = 0; i < nfine; ++i) kappa[i] = eta_c + h * (i - 0.5 * (nfine - 1));   // nfine even: eta_c mid-way
-    st = scan_line(plan, dir, pol, comp, k0, kappa, tol, xi, &warn);
-    if (st < 0) return st;
-    st = gsm_pole_search(nfine, kappa.data(), xi.data(), Np, Nd, kappa.front(), kappa.back(), eta, zeta, &best);
-    if (st < 0 || best < 0) return fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: no pole inside the fine window");
-    const double nr = eta[2 * best] / k0, ni = eta[2 * best + 1] / k0;
-    out[0] = nr; out[1] = ni;
-    out[2] = nr * nr - ni * ni; out[3] = 2.0 * nr * ni;
-    out[4] = zeta[2 * best]; out[5] = zeta[2 * best + 1];
-    return warn ? GSM_NOT_CONVERGED : GSM_OK;
+    if (!dir || !pol || !out) return plan ? fail(plan, GSM_E_INVALID, "gsm_retrieve_neff: bad argument") : GSM_E_INVALID;
+    return gsm_retrieve_neff_many(plan, 1, dir, pol, &comp, &k0, &n_lo, &n_hi, ncoarse, nfine, fine_step, tol, out, nullptr);
 }

@@ -12,7 +12,7 @@ namespace gsm {
 // Kernel classes for launch counting and (optional) per-class CUDA-event timing (gsm_plan_profile).
 enum KernelClass {
     KC_Z_FORWARD = 0, KC_XY_CONV, KC_Z_INVERSE_GREEN, KC_SWEEP_DOTS, KC_HSOLVE, KC_SWEEP_UPDATE, KC_GIVENS,
-    KC_NORMALIZE, KC_ARNOLDI_MGS, KC_COMBINE, KC_RESIDUAL, KC_SMALL, KC_PLAN, KC_COUNT
+    KC_NORMALIZE, KC_ARNOLDI_MGS, KC_COMBINE, KC_RESIDUAL, KC_SMALL, KC_PLAN, KC_APPLY_FUSED, KC_COUNT
 };
 const char* kernel_class_name(int cls);
 
@@ -45,7 +45,6 @@ struct ApplyGeom {
     int NL;              // N1*N2 = number of z-lines per component
     long n;              // N1*N2*N3
     int hform;           // 0: Eq. 4 (E, Green dyadic); 1: Eq. 5 (H, cross products around the Toeplitz product)
-    int sub;             // solves per pass through the workspace W (L2-resident sub-batches)
     int L;               // z-lines per CTA in passes 1 and 3
     int Lst;             // odd row stride (>= L) of the pass-1 tile
     int RS3;             // odd row stride (>= 3L) of the pass-3 tile
@@ -68,11 +67,34 @@ struct KrylovDims {
     int ld;          // mmax + 1
 };
 
+// Device state of the fused persistent apply for 64-point axes (apply_fused64.cu); ring == null: not in use.
+struct Fused64Dev {
+    int* head = nullptr;        // [1] ticket counter
+    int* cnt = nullptr;         // [3][maxB] per-solve completion counters of the three item kinds
+    int* nact = nullptr;        // [1] number of listed solves
+    int* list = nullptr;        // [maxB] batch indices of the solves of this launch
+    const int* items = nullptr; // [items per slot] slot pattern
+    cplx* ring = nullptr;       // W ring: [F64_RING][3][64][NL]
+    int maxB = 0, grid = 0;     // counters' stride; persistent grid size (CTAs)
+};
+
 // ---- launches implemented in apply.cu --------------------------------------------------------------------------
-// y[b] = x[b] - G_b (T x[b]); kvec[b][3], k0[b] device arrays; W workspace [batch][3][P3][NL].
-// active (may be null): per-solve flags; CTAs of solves with active[b] == 0 exit at once.
+// y[b] = x[b] - G_b (T x[b]); kvec[b][3], k0[b] device arrays; W workspace [batch][3][P3][NL] (three-launch path) or
+// `fused` (one persistent launch, 64-point axes).  active (may be null): per-solve flags; solves with active[b] == 0
+// are skipped.  units = number of solves whose algorithmic bytes are billed to the profiler now (run_batch bills the
+// iteration loop afterwards from the final iteration counts and passes 0).
 cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
-                         cplx* d_y, cplx* d_W, const int* d_active, cudaStream_t st, Profiler* prof, int nact);
+                         cplx* d_y, cplx* d_W, const Fused64Dev* fused, const int* d_active, cudaStream_t st,
+                         Profiler* prof, double units);
+// algorithmic bytes of `units` solve-applies (per-launch terms excluded) added to the apply's kernel classes
+void bill_apply(const ApplyGeom& g, bool fused, Profiler* prof, double units);
+// apply_fused64.cu
+size_t fused64_ring_elems(const ApplyGeom& g);
+int fused64_items_per_slot(const ApplyGeom& g);
+void fused64_slot_pattern(const ApplyGeom& g, int* items);
+cudaError_t apply_fused64_init_attributes(int* grid_out);
+cudaError_t launch_apply_fused64(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
+                                 cplx* d_y, const int* d_active, const Fused64Dev& f, cudaStream_t st);
 size_t apply_smem_max(const ApplyGeom& g);
 cudaError_t apply_init_attributes();
 // apply128.cu: pass 2 specialised for 128-point x and y axes
@@ -123,7 +145,9 @@ struct KrylovState {   // all device pointers, one entry (or row) per solve of t
     cplx* g;           // [batch][ld]
     cplx* ycoef;       // [batch][mmax]
     double* hist;      // [batch][mmax]
-    double* beta;      // [batch]
+    double* beta;      // [batch] ||r0||: norm of the first basis vector's unnormalised form
+    double* bnorm;     // [batch] ||b||: the stop test and the reported residuals are relative to it
+    int* guess;        // [batch] 1 when the solve starts from an initial guess x0 (r0 = b - A x0, x = x0 + d)
     double* scale;     // [batch] 1 / h_{j+1,j} of the running iteration
     int* active;       // [batch] 1 while iterating
     int* iters;        // [batch]
@@ -133,13 +157,27 @@ struct KrylovState {   // all device pointers, one entry (or row) per solve of t
 };
 cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0 /*index of m=0*/, long n,
                                cudaStream_t st, Profiler* prof);
-cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
 cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
-cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
 cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
-cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact);
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
 cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);
-cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st, Profiler* prof);
+// E[b] = (guess[b] ? x0[b] : 0) + sum_i y_i v_i; x0 may be null and may alias d_E
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_x0, cplx* d_E, cudaStream_t st,
+                           Profiler* prof);
+// Start from an initial guess (Saad Alg. 6.9 with x0 != 0): given y = A x0 in basis slot 1, set
+// r0 = b - y, beta = ||r0||, v_0 = r0 / beta, g_0 = beta for every solve whose guess beats the zero start
+// (||r0|| < ||b||); the others keep the state launch_krylov_init gave them.
+cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st,
+                                Profiler* prof);
+// scan over an ordered mesh (gsm_scan_mesh): guesses by interpolation of already solved neighbours, and the scatter
+// of a wave's solutions into the mesh-ordered field array.  nbr[b][4] = neighbour point indices (-1: unused),
+// wgt[b][4] their (complex) weights, idx[b] = point index of solve b.
+cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all, const int* d_nbr, const cplx* d_wgt,
+                              cplx* d_x0, cudaStream_t st, Profiler* prof);
+cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,
+                                cudaStream_t st, Profiler* prof);
 // resid[b] = || pol delta_m0 - y[b] || / beta[b]
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
                                  double* d_resid, cudaStream_t st, Profiler* prof);
@@ -150,6 +188,6 @@ cudaError_t krylov_init_attributes();
 // arnoldi_cluster_plan: cluster size (0 = not usable: fall back to the two-sweep kernels) and elements per CTA.
 cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_out, int* nclusters_out);
 cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, int batch, int j, int cs, int chunk,
-                                   int nclusters, cudaStream_t st, Profiler* prof, int nact);
+                                   int nclusters, cudaStream_t st, Profiler* prof);
 
 }  // namespace gsm

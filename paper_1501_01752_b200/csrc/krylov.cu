@@ -30,6 +30,8 @@ __global__ void krylov_init_kernel(KrylovDims d, KrylovState s, int batch, long 
     const double* p = s.pol + 6 * b;
     const double beta = sqrt(p[0] * p[0] + p[1] * p[1] + p[2] * p[2] + p[3] * p[3] + p[4] * p[4] + p[5] * p[5]);
     s.beta[b] = beta;
+    s.bnorm[b] = beta;
+    s.guess[b] = 0;
     s.iters[b] = 0;
     s.active[b] = beta > 0.0 ? 1 : 0;
     if (beta <= 0.0) atomicSub(s.nactive, 1);
@@ -244,9 +246,9 @@ __global__ void backsolve_kernel(KrylovDims d, KrylovState s, int batch) {
     }
 }
 
-// E[b] = sum_{i<m} y_i v_i
+// E[b] = x0[b] (if the solve started from a guess) + sum_{i<m} y_i v_i.  x0 may alias out (same thread, same element).
 template <int E>
-__global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s, int batch, cplx* __restrict__ out) {
+__global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s, int batch, const cplx* x0, cplx* out) {
     const int b = blockIdx.y;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* y = reinterpret_cast<cplx*>(smem_raw);
@@ -257,8 +259,12 @@ __global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s
     const long vs = (long)batch * d.vlen;
     const cplx* vb = s.basis + (long)b * d.vlen;
     cplx acc[E];
+    const bool g0 = x0 != nullptr && s.guess[b] != 0;
 #pragma unroll
-    for (int k = 0; k < E; ++k) acc[k] = make_double2(0.0, 0.0);
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        acc[k] = (g0 && e < d.vlen) ? x0[(long)b * d.vlen + e] : make_double2(0.0, 0.0);
+    }
     for (int i = 0; i < m; ++i) {
         const cplx* vi = vb + (long)i * vs;
         const cplx yi = y[i];
@@ -275,10 +281,10 @@ __global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s
     }
 }
 
-// partial ||b - y||^2 per chunk, b = pol delta_{m,0}
+// partial ||b - y||^2 per chunk, b = pol delta_{m,0}; r_out (may be null) receives b - y
 template <int E>
 __global__ void __launch_bounds__(KT) resid_part_kernel(KrylovDims d, KrylovState s, int batch, const cplx* __restrict__ y,
-                                                        long i0, long n) {
+                                                        long i0, long n, cplx* __restrict__ r_out) {
     const int b = blockIdx.y;
     __shared__ double wsum[KT / 32];
     const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
@@ -290,6 +296,7 @@ __global__ void __launch_bounds__(KT) resid_part_kernel(KrylovDims d, KrylovStat
             cplx v = y[(long)b * d.vlen + e];
             const long c = e / n, r = e - c * n;
             if (r == i0) { v.x -= s.pol[6 * b + 2 * c]; v.y -= s.pol[6 * b + 2 * c + 1]; }
+            if (r_out) r_out[(long)b * d.vlen + e] = make_double2(-v.x, -v.y);
             nn = fma(v.x, v.x, fma(v.y, v.y, nn));
         }
     }
@@ -307,7 +314,84 @@ __global__ void resid_final_kernel(KrylovDims d, KrylovState s, int batch, doubl
     if (b >= batch) return;
     double nn = 0.0;
     for (int c = 0; c < d.nchunk; ++c) nn += s.part[(long)b * 2 * d.ld * d.nchunk + c].x;
-    resid[b] = s.beta[b] > 0.0 ? sqrt(nn) / s.beta[b] : 0.0;
+    resid[b] = s.bnorm[b] > 0.0 ? sqrt(nn) / s.bnorm[b] : 0.0;
+}
+
+// initial guess, per solve: beta = ||r0|| from the chunk partials; the guess is taken when it beats the zero start
+__global__ void guess_init_kernel(KrylovDims d, KrylovState s, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    double nn = 0.0;
+    for (int c = 0; c < d.nchunk; ++c) nn += s.part[(long)b * 2 * d.ld * d.nchunk + c].x;
+    const double beta = sqrt(nn), bn = s.bnorm[b];
+    if (!(bn > 0.0) || !(beta < bn)) return;      // zero source, or a guess worse than x0 = 0: keep the zero start
+    s.guess[b] = 1;
+    s.beta[b] = beta;
+    s.g[(long)b * d.ld] = make_double2(beta, 0.0);
+    if (beta <= s.tol[0] * bn) {                  // the guess already meets the stop test: no iteration
+        s.active[b] = 0;
+        atomicSub(s.nactive, 1);
+    }
+}
+// v_0 = r0 / beta for the solves that took their guess (r0 sits in basis slot 0 already, unnormalised)
+template <int E>
+__global__ void __launch_bounds__(KT) guess_v0_kernel(KrylovDims d, KrylovState s, int batch, long i0, long n) {
+    const int b = blockIdx.y;
+    const bool g = s.guess[b] != 0;
+    const double sc = g ? 1.0 / s.beta[b] : 0.0, bn = s.bnorm[b];
+    cplx* v0 = s.basis + (long)b * d.vlen;
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e >= d.vlen) continue;
+        if (g) {
+            const cplx v = v0[e];
+            v0[e] = make_double2(v.x * sc, v.y * sc);
+        } else {                                  // zero start: v_0 = b / ||b|| (the delta vector of launch_krylov_init)
+            const long c = e / n, r = e - c * n;
+            v0[e] = (r == i0 && bn > 0.0) ? make_double2(s.pol[6 * b + 2 * c] / bn, s.pol[6 * b + 2 * c + 1] / bn)
+                                          : make_double2(0.0, 0.0);
+        }
+    }
+}
+
+// x0[b] = sum_q wgt[b][q] all[nbr[b][q]]  (interpolation of solved neighbours along the mesh, complex weights)
+template <int E>
+__global__ void __launch_bounds__(KT) mesh_guess_kernel(KrylovDims d, const cplx* __restrict__ all, const int* __restrict__ nbr,
+                                                        const cplx* __restrict__ wgt, cplx* __restrict__ x0) {
+    const int b = blockIdx.y;
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    cplx acc[E];
+#pragma unroll
+    for (int k = 0; k < E; ++k) acc[k] = make_double2(0.0, 0.0);
+    for (int q = 0; q < 4; ++q) {
+        const int p = nbr[4 * b + q];
+        if (p < 0) continue;
+        const cplx w = wgt[4 * b + q];
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            const long e = e0 + (long)k * KT;
+            if (e < d.vlen) acc[k] = cfma(w, all[(long)p * d.vlen + e], acc[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) x0[(long)b * d.vlen + e] = acc[k];
+    }
+}
+template <int E>
+__global__ void __launch_bounds__(KT) mesh_scatter_kernel(KrylovDims d, const cplx* __restrict__ src, const int* __restrict__ idx,
+                                                          cplx* __restrict__ all) {
+    const int b = blockIdx.y;
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+    cplx* dst = all + (long)idx[b] * d.vlen;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e < d.vlen) dst[e] = src[(long)b * d.vlen + e];
+    }
 }
 
 // ---- host-side launchers ----------------------------------------------------------------------------------------
@@ -323,8 +407,11 @@ cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int ba
     krylov_init_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, i0, n);
     return cudaGetLastError();
 }
-cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
-    ProfScope ps_(prof, KC_SWEEP_DOTS, st, 16.0 * d.vlen * (j + 2.0) * nact);   // reads w and v_0..v_j
+// The sweeps' algorithmic bytes depend on how many solves are still iterating, which the host does not know at launch
+// time: run_batch bills them afterwards from the final iteration counts (sweep_dots (j+2) V: w and v_0..v_j;
+// sweep_update (j+3) V: w, v_0..v_j, write w; normalize 2 V).
+cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SWEEP_DOTS, st);
     const size_t smem = sizeof(double) * 4 * (KT / 32) * (size_t)(j + 1);
     sweep_dots_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, smem, st>>>(d, s, batch, j);
     return cudaGetLastError();
@@ -337,8 +424,8 @@ cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, 
     hsolve_kernel<<<batch, HS_T, smem, st>>>(d, s, batch, j, stage);
     return cudaGetLastError();
 }
-cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
-    ProfScope ps_(prof, KC_SWEEP_UPDATE, st, 16.0 * d.vlen * (j + 3.0) * nact);   // reads w, v_0..v_j; writes w
+cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SWEEP_UPDATE, st);
     sweep_update_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * (j + 1), st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
@@ -347,8 +434,8 @@ cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, 
     givens_kernel<<<batch, 32, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof, int nact) {
-    ProfScope ps_(prof, KC_NORMALIZE, st, 16.0 * d.vlen * 2.0 * nact);
+cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_NORMALIZE, st);
     normalize_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
@@ -357,15 +444,40 @@ cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batc
     backsolve_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch);
     return cudaGetLastError();
 }
-cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, cplx* d_E, cudaStream_t st, Profiler* prof) {
-    ProfScope ps_(prof, KC_COMBINE, st, 16.0 * d.vlen * batch * (d.mmax / 2 + 1.0));
-    combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_E);
+cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st,
+                                Profiler* prof) {
+    const cplx* y = s.basis + (size_t)batch * d.vlen;   // slot 1 holds A x0
+    cplx* r0 = s.basis;                                 // slot 0 receives b - A x0, then v_0
+    { ProfScope ps_(prof, KC_RESIDUAL, st);
+      resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, y, i0, n, r0); }
+    { ProfScope ps_(prof, KC_SMALL, st);
+      guess_init_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch); }
+    ProfScope ps_(prof, KC_NORMALIZE, st);
+    guess_v0_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, i0, n);
+    return cudaGetLastError();
+}
+cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all, const int* d_nbr, const cplx* d_wgt,
+                              cplx* d_x0, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
+    mesh_guess_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, d_all, d_nbr, d_wgt, d_x0);
+    return cudaGetLastError();
+}
+cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,
+                                cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
+    mesh_scatter_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, d_src, d_idx, d_all);
+    return cudaGetLastError();
+}
+cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_x0, cplx* d_E, cudaStream_t st,
+                           Profiler* prof) {
+    ProfScope ps_(prof, KC_COMBINE, st);   // (m_b + 1) V per solve, billed by run_batch from the iteration counts
+    combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_x0, d_E);
     return cudaGetLastError();
 }
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
                                  double* d_resid, cudaStream_t st, Profiler* prof) {
     { ProfScope ps_(prof, KC_RESIDUAL, st);
-    resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, d_y, i0, n); }
+    resid_part_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, d_y, i0, n, nullptr); }
     ProfScope ps2_(prof, KC_SMALL, st);
     resid_final_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch, d_resid);
     return cudaGetLastError();

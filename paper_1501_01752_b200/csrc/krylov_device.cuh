@@ -39,7 +39,7 @@ __device__ __forceinline__ void givens_step(const KrylovDims& d, const KrylovSta
     g[j + 1] = gn;
     g[j] = make_double2(c * gj.x, c * gj.y);
     const double beta = s.beta[b];
-    const double res = hypot(gn.x, gn.y) / beta;
+    const double res = hypot(gn.x, gn.y) / s.bnorm[b];
     s.hist[(long)b * d.mmax + j] = res;
     s.iters[b] = j + 1;
     const bool lucky = hn <= 2.220446049250313e-16 * beta;

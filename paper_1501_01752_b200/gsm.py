@@ -18,6 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libgsm_b200.so")
 OK, NOT_CONVERGED, E_INVALID, E_ALLOC, E_CUDA, E_SINGULAR_BASIS = 0, 1, -1, -2, -3, -4
 SPHERE, ELLIPSOID, BOX = 0, 1, 2
 FORM_E, FORM_H = 0, 1
+FLAG_TWO_SWEEP, FLAG_GENERIC_APPLY, FLAG_FUSED_APPLY = 1, 2, 4   # diagnostics (include/gsm.h GSM_FLAG_*)
+MAX_ITERS = 512
 
 
 class GsmError(RuntimeError):
@@ -38,7 +40,7 @@ class _PlanDesc(C.Structure):
                 ("n_shapes", C.c_int), ("shapes", C.POINTER(_Shape)),
                 ("voxels", C.c_int * 3), ("eps_grid_host", C.c_void_p),
                 ("max_iters", C.c_int), ("max_batch", C.c_int), ("cuda_stream", C.c_void_p),
-                ("formulation", C.c_int)]
+                ("formulation", C.c_int), ("flags", C.c_int)]
 
 
 def _load():
@@ -56,6 +58,8 @@ def _load():
     lib.gsm_apply.argtypes = [P, C.c_int, P, P, P, P]
     lib.gsm_solve.argtypes = [P, P, C.c_double, P, C.c_double, P, P, C.c_int, ip, dp]
     lib.gsm_scan.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P]
+    lib.gsm_scan_guess.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P, P]
+    lib.gsm_scan_mesh.argtypes = [P, C.c_int, P, P, P, C.c_double, C.c_int, P, P, P, P]
     lib.gsm_pole_search.argtypes = [C.c_int, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P, ip]
     lib.gsm_plan_set_cell.argtypes = [P, C.POINTER(_PlanDesc)]
     lib.gsm_plan_profile.argtypes = [P, C.c_int]
@@ -67,10 +71,13 @@ def _load():
     lib.gsm_retrieve_neff.argtypes = [P, P, P, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
                                       C.c_double, P]
     lib.gsm_retrieve_neff.restype = C.c_int
+    lib.gsm_retrieve_neff_many.argtypes = [P, C.c_int, P, P, P, P, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P]
+    lib.gsm_retrieve_neff_many.restype = C.c_int
     lib.gsm_last_error.argtypes = [P]
     lib.gsm_last_error.restype = C.c_char_p
     for f in ("gsm_plan_create", "gsm_plan_destroy", "gsm_plan_coeffs", "gsm_plan_info", "gsm_apply", "gsm_solve",
-              "gsm_scan", "gsm_pole_search", "gsm_plan_set_cell", "gsm_plan_profile", "gsm_plan_profile_read"):
+              "gsm_scan", "gsm_scan_guess", "gsm_scan_mesh", "gsm_pole_search", "gsm_plan_set_cell", "gsm_plan_profile",
+              "gsm_plan_profile_read"):
         getattr(lib, f).restype = C.c_int
     return lib
 
@@ -95,13 +102,14 @@ class Plan:
     """gsm_plan: one periodic cell (periods, orders, shapes or voxel grid) on the current CUDA device."""
 
     def __init__(self, periods, orders, shapes=None, eps_bg=1.0, eps_b=None, voxels=None, max_iters=64, max_batch=1,
-                 stream=None, formulation=FORM_E):
+                 stream=None, formulation=FORM_E, flags=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1501_01752_b200.gsm needs a CUDA device; there is no CPU fallback")
         self._torch = torch
         self.stream = stream
         self.formulation = int(formulation)
+        self.flags = int(flags)
         self.orders = tuple(int(n) for n in orders)
         d, keep = self._desc(periods, shapes, eps_bg, eps_b, voxels, max_iters, max_batch)
         self.n = int(np.prod(self.orders))
@@ -148,6 +156,7 @@ class Plan:
         d.max_iters, d.max_batch = int(max_iters), int(max_batch)
         d.cuda_stream = self.stream.cuda_stream if self.stream is not None else None
         d.formulation = self.formulation
+        d.flags = self.flags
         return d, keep
 
     def set_cell(self, periods, shapes=None, eps_bg=1.0, eps_b=None, voxels=None):
@@ -196,13 +205,24 @@ class Plan:
 
     # -- hot path -------------------------------------------------------------------------------------------
     def apply(self, k_bloch, k0, x, out=None):
-        """gsm_apply: y = x - G (T x).  x: cuda complex128 tensor [batch, 3, N1, N2, N3]; asynchronous."""
+        """gsm_apply: y = x - G (T x).  x: cuda complex128 tensor [batch, 3, N1, N2, N3].
+
+        Asynchronous on the plan's stream; ordered after the work already queued on torch's current stream (which
+        produced x) and before whatever the current stream does next (which may read y)."""
         torch = self._torch
         batch = x.shape[0]
         assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous() and tuple(x.shape[1:]) == (3,) + self.orders
         y = torch.empty_like(x) if out is None else out
         kb, kk = _f64(k_bloch, (batch, 3)), _f64(k0, (batch,))
+        cur = torch.cuda.current_stream()
+        side = self.stream is not None and self.stream != cur
+        if side:
+            self.stream.wait_stream(cur)
         _check(_lib.gsm_apply(self._h, batch, kb.ctypes.data, kk.ctypes.data, x.data_ptr(), y.data_ptr()), self._h)
+        if side:
+            cur.wait_stream(self.stream)
+            x.record_stream(self.stream)
+            y.record_stream(self.stream)
         return y
 
     def solve(self, k_bloch, k0, pol, tol=1e-10, out=None):
@@ -217,11 +237,13 @@ class Plan:
                                    hist.ctypes.data, self.max_iters, C.byref(it), C.byref(res)), self._h)
         return E, hist[: it.value].copy(), it.value, res.value, st
 
-    def scan(self, k_bloch, k0, pol, tol=1e-10, fields=None):
+    def scan(self, k_bloch, k0, pol, tol=1e-10, fields=None, x0=None, levels=None):
         """gsm_scan: returns (resp [npts,3] complex, iters [npts], resid [npts], status).
 
         pol: [npts, 6] real (interleaved complex) or [npts, 3] complex.  fields: optional cuda tensor
-        [npts, 3, N1, N2, N3] that receives every solution."""
+        [npts, 3, N1, N2, N3] that receives every solution.  x0: optional cuda tensor of the same shape with initial
+        guesses (gsm_scan_guess; may be `fields` itself).  levels: solve the list as an ordered equidistant mesh in
+        that many coarse-to-fine waves, each started from the interpolation of the previous ones (gsm_scan_mesh)."""
         kb = _f64(k_bloch)
         npts = kb.shape[0]
         kk = _f64(k0, (npts,))
@@ -232,10 +254,19 @@ class Plan:
         resp = np.zeros((npts, 3), dtype=np.complex128)
         iters = np.zeros(npts, dtype=np.int32)
         resid = np.zeros(npts)
-        st = _check(_lib.gsm_scan(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol),
-                                  resp.ctypes.data, iters.ctypes.data, resid.ctypes.data,
-                                  fields.data_ptr() if fields is not None else None), self._h)
-        return resp, iters, resid, st
+        fp = fields.data_ptr() if fields is not None else None
+        if levels is not None:
+            assert x0 is None
+            st = _lib.gsm_scan_mesh(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol), int(levels),
+                                    resp.ctypes.data, iters.ctypes.data, resid.ctypes.data, fp)
+        elif x0 is not None:
+            assert x0.is_cuda and x0.is_contiguous() and tuple(x0.shape) == (npts, 3) + self.orders
+            st = _lib.gsm_scan_guess(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol),
+                                     x0.data_ptr(), resp.ctypes.data, iters.ctypes.data, resid.ctypes.data, fp)
+        else:
+            st = _lib.gsm_scan(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol),
+                               resp.ctypes.data, iters.ctypes.data, resid.ctypes.data, fp)
+        return resp, iters, resid, _check(st, self._h)
 
 
     def retrieve_neff(self, direction, pol, comp, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):
@@ -247,6 +278,25 @@ class Plan:
                                            float(n_hi), int(ncoarse), int(nfine), float(fine_step), float(tol),
                                            out.ctypes.data), self._h)
         return complex(out[0], out[1]), complex(out[2], out[3]), complex(out[4], out[5]), st
+
+
+    def retrieve_neff_many(self, directions, pols, comps, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):
+        """gsm_retrieve_neff_many: nlines retrievals with every stage in one scan.  directions [n,3]; pols [n,3] complex;
+        comps [n] (component index, or -1 = projection on the amplitude); k0, n_lo, n_hi scalars or [n].
+        Returns (n_eff [n] complex, eps_eff [n] complex, zeta [n] complex, line_status [n], status)."""
+        d = _f64(directions)
+        n = d.shape[0]
+        pl = _f64(np.ascontiguousarray(pols, dtype=np.complex128).view(np.float64), (n, 6))
+        cp = np.ascontiguousarray(np.broadcast_to(np.asarray(comps, dtype=np.int32), (n,)))
+        kk, lo, hi = (_f64(np.broadcast_to(np.asarray(v, dtype=np.float64), (n,))) for v in (k0, n_lo, n_hi))
+        out = np.zeros((n, 6))
+        ls = np.full(n, E_INVALID, dtype=np.int32)
+        st = _lib.gsm_retrieve_neff_many(self._h, n, d.ctypes.data, pl.ctypes.data, cp.ctypes.data, kk.ctypes.data,
+                                         lo.ctypes.data, hi.ctypes.data, int(ncoarse), int(nfine), float(fine_step),
+                                         float(tol), out.ctypes.data, ls.ctypes.data)
+        if st < 0 and not np.any(ls == OK):
+            _check(st, self._h)
+        return out[:, 0] + 1j * out[:, 1], out[:, 2] + 1j * out[:, 3], out[:, 4] + 1j * out[:, 5], ls, st
 
 
 def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):
@@ -265,7 +315,7 @@ def pole_search(kappa, xi, Np=5, Nd=10, lo=None, hi=None):
     return eta, zeta, best.value
 
 
-def plan_from_geometry(geo, max_iters=64, max_batch=1, stream=None, formulation=FORM_E) -> Plan:
+def plan_from_geometry(geo, max_iters=64, max_batch=1, stream=None, formulation=FORM_E, flags=0) -> Plan:
     """Plan for a workloads.Geometry (seeded input description; holds no arithmetic of the method)."""
     return Plan(geo.periods, geo.orders, shapes=geo.shapes, eps_bg=geo.eps_bg, eps_b=geo.eps_b, voxels=geo.voxels,
-                max_iters=max_iters, max_batch=max_batch, stream=stream, formulation=formulation)
+                max_iters=max_iters, max_batch=max_batch, stream=stream, formulation=formulation, flags=flags)

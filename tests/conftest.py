@@ -27,9 +27,14 @@ def _oracle_helper():
     build_oracle()
 
 
-def load_golden():
+def load_oracle_golden():
+    """tests/golden/oracle_neff.txt: values written by tests/golden/make_oracle_goldens.py from the oracle alone."""
+    return load_golden("oracle_neff.txt")
+
+
+def load_golden(name="paper_values.txt"):
     vals = {}
-    with open(os.path.join(ROOT, "tests", "golden", "paper_values.txt")) as f:
+    with open(os.path.join(ROOT, "tests", "golden", name)) as f:
         for line in f:
             line = line.split("#")[0].strip()
             if line:

@@ -212,4 +212,8 @@ def test_launch_accounting_and_event_profile():
     assert iters <= steps <= iters + 1
     assert all(ms > 0 for (n, ms, by) in pr.values() if n > 0)
     assert pr["xy_conv"][2] > 0 and plan.info()["launches"] == 0       # bytes were accounted; the reset cleared the counters
+    # algorithmic bytes are billed from the final iteration count m: the Arnoldi step of iteration j moves (j + 3) V
+    V, m = 16.0 * 3 * geo.n, iters
+    if pr["arnoldi_mgs"][0]:
+        assert pr["arnoldi_mgs"][2] == V * (m * (m - 1) / 2 + 3 * m)
     plan.close()

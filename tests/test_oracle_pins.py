@@ -383,3 +383,27 @@ def test_two_stage_retrieval_synthetic_pole_and_uniform_cell():
                                                         [1.0, 0, 0]))[0] for kv in kappa])
     n, eps, _ = orc.retrieve_two_stage(xi_cell, k0, 1.3, 1.8)
     assert abs(eps - eps2) <= 1e-9 and abs(n - np.sqrt(eps2)) <= 1e-9
+
+
+def test_gmres_with_initial_guess():
+    """gmres(x0=...) (Saad Alg. 6.9 with a non-zero start): same solution as dense LU whatever the guess;
+    the exact solution as guess takes no iteration; the neighbouring kappa point's field as guess takes fewer iterations
+    than the zero start; the history stays relative to ||b||."""
+    g = W.sphere_lattice((5, 5, 5))
+    c = coeffs(g)
+    kb, kb2 = np.array([0.0, 0.0, 1.12 * K0]), np.array([0.0, 0.0, 1.125 * K0])
+    pol = [1.0, 0.2j, 0.0]
+    ref = O.solve_dense(c, g.periods, g.orders, kb, K0, 1.0, pol)
+    nb = O.solve_dense(c, g.periods, g.orders, kb2, K0, 1.0, pol)
+    E0, h0, m0 = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-12)
+    rnd = W.random_field(1, g.orders)[0]
+    for x0 in (nb, rnd, 3.0 * ref):
+        E, h, m = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-12, x0=x0)
+        assert np.linalg.norm(E - ref) / np.linalg.norm(ref) < 1e-10
+        assert h[-1] <= 1e-12 and np.all(np.diff(h) <= 1e-15)
+        r = O.incident(g.orders, pol) - O.apply_operator(c, E, g.periods, kb, K0, 1.0)
+        assert abs(np.linalg.norm(r) / np.linalg.norm(O.incident(g.orders, pol)) - h[-1]) < 1e-12   # estimate = true, / ||b||
+    E, h, m = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-12, x0=nb)
+    assert m < m0
+    E, h, m = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-10, x0=ref)
+    assert m == 0 and h == [] and np.array_equal(E, ref)
