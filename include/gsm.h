@@ -45,7 +45,7 @@ typedef enum {
     GSM_E_SINGULAR_BASIS = -4  /* min_m |k_m.k_m - k_b^2| / |k_b^2| < 1e-12: eps_b violates PAPER.md:52       */
 } gsm_status;
 
-enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2 };
+enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2, GSM_POLYHEDRON = 3 };
 
 /* Formulation solved by the plan.
  *   GSM_FORM_E: Eq. 4, unknown E, coefficients c_d = ((eps - eps_b)/eps_b)_d            (the default)
@@ -69,12 +69,21 @@ enum { GSM_FLAG_TWO_SWEEP = 1, GSM_FLAG_GENERIC_APPLY = 2, GSM_FLAG_FUSED_APPLY 
 /* One analytic inclusion ("Fourier images of sphere and polyhedron can be combined").
  * size = (R, -, -) for a sphere, semi-axes for an ellipsoid, full edge lengths for an axis-aligned box; same
  * length unit as the periods.  The inclusion's permittivity replaces the background inside it; overlapping
- * inclusions superpose their (eps_i - eps_bg) contrasts. */
+ * inclusions superpose their (eps_i - eps_bg) contrasts.
+ * GSM_POLYHEDRON: any closed polyhedron with planar faces, convex or not (size unused).  vertices[n_vertices][3] are
+ * given relative to center; face f lists face_sizes[f] >= 3 vertex indices, consecutively in face_vertices, counter-
+ * clockwise seen from outside.  Its Fourier image is evaluated in closed form (divergence theorem: faces, then edges).
+ * The arrays are host memory, read before gsm_plan_create / gsm_plan_set_cell return. */
 typedef struct {
     int kind;
     double center[3];
     double size[3];
     double eps_re, eps_im;
+    int n_vertices;
+    const double* vertices;
+    int n_faces;
+    const int* face_sizes;
+    const int* face_vertices;
 } gsm_shape;
 
 /* Plan descriptor.  Exactly one of (n_shapes > 0, shapes) or (eps_grid_host != NULL) describes the cell.

@@ -28,7 +28,7 @@ import os
 
 import numpy as np
 
-SPHERE, ELLIPSOID, BOX = 0, 1, 2
+SPHERE, ELLIPSOID, BOX, POLYHEDRON = 0, 1, 2, 3
 
 
 # --------------------------------------------------------------------------------------------------
@@ -69,11 +69,53 @@ def _sinc(t: np.ndarray) -> np.ndarray:
     return out
 
 
+def polyhedron_image(G, vertices, faces) -> complex:
+    """int_P exp(-i G.r) d^3r for a polyhedron with planar faces ("Fourier images of sphere and
+    polyhedron"; the paper prints no formula - this is the divergence theorem applied twice, textbook):
+
+        G != 0:  (i / |G|^2) sum_faces (G.n_f) I_f,            I_f = int_face exp(-i G.r) dS
+        I_f   =  (i / |G_t|^2) sum_edges (G_t.m_e) L_e exp(-i G.c_e) sinc(G.(b - a) / 2)      if G_t != 0
+              =  A_f exp(-i G.r_f)                                                            if G_t = 0
+    with n_f the outward unit normal, G_t = G - (G.n_f) n_f, and for every edge a -> b of the face (vertices listed
+    counter-clockwise seen from outside): length L_e, midpoint c_e, in-plane outward normal m_e = t_e x n_f.
+    G = 0 gives the volume, (1/3) sum_faces (r_f.n_f) A_f."""
+    G = np.asarray(G, dtype=np.float64)
+    V = np.asarray(vertices, dtype=np.float64)
+    g2 = float(G @ G)
+    total = 0.0 + 0.0j
+    for f in faces:
+        P = V[list(f)]
+        nvec = np.zeros(3)
+        for k in range(1, len(P) - 1):                           # area vector of the fan triangulation
+            nvec += 0.5 * np.cross(P[k] - P[0], P[k + 1] - P[0])
+        area = float(np.linalg.norm(nvec))
+        n = nvec / area
+        if g2 == 0.0:
+            total += float(P[0] @ n) * area / 3.0
+            continue
+        Gn = float(G @ n)
+        Gt = G - Gn * n
+        gt2 = float(Gt @ Gt)
+        if gt2 < 1e-18 * g2:
+            If = area * np.exp(-1j * float(G @ P[0]))
+        else:
+            If = 0.0 + 0.0j
+            for k in range(len(P)):
+                a, b = P[k], P[(k + 1) % len(P)]
+                L = float(np.linalg.norm(b - a))
+                m = np.cross((b - a) / L, n)
+                If += float(Gt @ m) * L * np.exp(-1j * float(G @ (a + b)) / 2) * np.sinc(float(G @ (b - a)) / 2 / np.pi)
+            If *= 1j / gt2
+        total += 1j / g2 * Gn * If
+    return complex(total)
+
+
 def coeffs_analytic(periods, orders, shapes, eps_bg=1.0, eps_b=None) -> np.ndarray:
     """c_d = (1/V) int_cell (eps(r)-eps_b)/eps_b exp(-i G_d.r) d^3r for superposed analytic shapes.
 
     shapes: list of dicts {kind, center(3), size(3), eps}.  size = (R, -, -) for a sphere, semi-axes for
-    an ellipsoid, full widths for a box.  c_d = delta_d0 (eps_bg-eps_b)/eps_b
+    an ellipsoid, full widths for a box; a polyhedron carries `vertices` (relative to the centre) and `faces`
+    (vertex index lists, counter-clockwise seen from outside) instead.  c_d = delta_d0 (eps_bg-eps_b)/eps_b
         + sum_i (eps_i-eps_bg)/eps_b * f_i * S_i(d) * exp(-i G_d.r_c,i).
     """
     eps_b = eps_bg if eps_b is None else eps_b
@@ -99,6 +141,11 @@ def coeffs_analytic(periods, orders, shapes, eps_bg=1.0, eps_b=None) -> np.ndarr
         elif kind == BOX:
             f = float(np.prod(size)) / vol
             S = _sinc(G1 * size[0] / 2) * _sinc(G2 * size[1] / 2) * _sinc(G3 * size[2] / 2)
+        elif kind == POLYHEDRON:                                 # vertices relative to the centre; f S = image / V_cell
+            f = 1.0 / vol
+            S = np.empty(G1.shape, dtype=np.complex128)
+            for idx in np.ndindex(G1.shape):
+                S[idx] = polyhedron_image((G1[idx], G2[idx], G3[idx]), s["vertices"], s["faces"])
         else:
             raise ValueError("unknown shape kind")
         phase = np.exp(-1j * (G1 * ctr[0] + G2 * ctr[1] + G3 * ctr[2]))

@@ -136,6 +136,55 @@ static cplx cdivh(double ar, double ai, double br, double bi) {
     return make_double2((ar * br + ai * bi) * inv, (ai * br - ar * bi) * inv);
 }
 
+// Polyhedron geometry for the device (plan_kernels.cu polyhedron_image): normals, areas, edges.  False if the
+// description is malformed (index out of range, degenerate face, fewer than 4 faces).
+static bool prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<PolyFace>& faces, std::vector<PolyEdge>& edges) {
+    if (s.n_vertices < 4 || s.n_faces < 4 || !s.vertices || !s.face_sizes || !s.face_vertices) return false;
+    q.f0 = (int)faces.size();
+    q.nf = s.n_faces;
+    q.vol = 0.0;
+    const int* fv = s.face_vertices;
+    for (int f = 0; f < s.n_faces; ++f) {
+        const int cnt = s.face_sizes[f];
+        if (cnt < 3) return false;
+        for (int k = 0; k < cnt; ++k)
+            if (fv[k] < 0 || fv[k] >= s.n_vertices) return false;
+        auto V = [&](int k) { return s.vertices + 3 * (size_t)fv[k % cnt]; };
+        PolyFace F{};
+        double nv[3] = {0.0, 0.0, 0.0};
+        for (int k = 1; k + 1 < cnt; ++k) {           // area vector of the fan triangulation
+            const double a[3] = {V(k)[0] - V(0)[0], V(k)[1] - V(0)[1], V(k)[2] - V(0)[2]};
+            const double b[3] = {V(k + 1)[0] - V(0)[0], V(k + 1)[1] - V(0)[1], V(k + 1)[2] - V(0)[2]};
+            nv[0] += 0.5 * (a[1] * b[2] - a[2] * b[1]);
+            nv[1] += 0.5 * (a[2] * b[0] - a[0] * b[2]);
+            nv[2] += 0.5 * (a[0] * b[1] - a[1] * b[0]);
+        }
+        F.area = std::sqrt(nv[0] * nv[0] + nv[1] * nv[1] + nv[2] * nv[2]);
+        if (!(F.area > 0.0)) return false;
+        for (int a = 0; a < 3; ++a) { F.n[a] = nv[a] / F.area; F.p0[a] = V(0)[a]; }
+        q.vol += (F.p0[0] * F.n[0] + F.p0[1] * F.n[1] + F.p0[2] * F.n[2]) * F.area / 3.0;
+        F.e0 = (int)edges.size();
+        F.ne = cnt;
+        for (int k = 0; k < cnt; ++k) {
+            PolyEdge E{};
+            double d[3];
+            for (int a = 0; a < 3; ++a) {
+                d[a] = V(k + 1)[a] - V(k)[a];
+                E.mid[a] = 0.5 * (V(k + 1)[a] + V(k)[a]);
+                E.half[a] = 0.5 * d[a];
+            }
+            // L m = L (t x n) = (b - a) x n
+            E.mL[0] = d[1] * F.n[2] - d[2] * F.n[1];
+            E.mL[1] = d[2] * F.n[0] - d[0] * F.n[2];
+            E.mL[2] = d[0] * F.n[1] - d[1] * F.n[0];
+            edges.push_back(E);
+        }
+        faces.push_back(F);
+        fv += cnt;
+    }
+    return q.vol > 0.0;
+}
+
 // a0: coefficients c_d on the device, either from closed forms or from an FFT of the voxel grid
 static gsm_status build_coeffs(gsm_plan* plan) {
     const gsm_plan_desc& d = plan->desc;
@@ -144,6 +193,8 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     if (!plan->coef) CK(dalloc(plan, &plan->coef, ncoef));
     if (d.eps_grid_host == nullptr) {
         std::vector<ShapeDev> hs(std::max(d.n_shapes, 1));
+        std::vector<PolyFace> pfaces;
+        std::vector<PolyEdge> pedges;
         const double vol = d.period[0] * d.period[1] * d.period[2];
         for (int i = 0; i < d.n_shapes; ++i) {
             const gsm_shape& s = d.shapes[i];
@@ -160,20 +211,34 @@ static gsm_status build_coeffs(gsm_plan* plan) {
             if (s.kind == GSM_SPHERE) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[0] * s.size[0] / vol;
             else if (s.kind == GSM_ELLIPSOID) q.f = 4.0 / 3.0 * M_PI * s.size[0] * s.size[1] * s.size[2] / vol;
             else if (s.kind == GSM_BOX) q.f = s.size[0] * s.size[1] * s.size[2] / vol;
-            else return fail(plan, GSM_E_INVALID, "unknown shape kind");
+            else if (s.kind == GSM_POLYHEDRON) {
+                q.f = 1.0 / vol;
+                if (!prepare_polyhedron(s, q, pfaces, pedges))
+                    return fail(plan, GSM_E_INVALID, "malformed polyhedron (indices, degenerate face, or inward orientation)");
+            } else return fail(plan, GSM_E_INVALID, "unknown shape kind");
         }
         ShapeDev* dsh = nullptr;
+        PolyFace* dfaces = nullptr;
+        PolyEdge* dedges = nullptr;
         CK(cudaMalloc(&dsh, sizeof(ShapeDev) * hs.size()));
         cudaError_t e = cudaMemcpyAsync(dsh, hs.data(), sizeof(ShapeDev) * hs.size(), cudaMemcpyHostToDevice, plan->stream);
+        if (e == cudaSuccess && !pfaces.empty()) {
+            e = cudaMalloc(&dfaces, sizeof(PolyFace) * pfaces.size());
+            if (e == cudaSuccess) e = cudaMalloc(&dedges, sizeof(PolyEdge) * pedges.size());
+            if (e == cudaSuccess) e = cudaMemcpyAsync(dfaces, pfaces.data(), sizeof(PolyFace) * pfaces.size(), cudaMemcpyHostToDevice, plan->stream);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(dedges, pedges.data(), sizeof(PolyEdge) * pedges.size(), cudaMemcpyHostToDevice, plan->stream);
+        }
         cplx c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_b_re, d.eps_b_im);
         if (d.formulation == GSM_FORM_H)     // 1 - eps_b/eps_bg = (eps_bg - eps_b)/eps_bg
             c0 = cdivh(d.eps_bg_re - d.eps_b_re, d.eps_bg_im - d.eps_b_im, d.eps_bg_re, d.eps_bg_im);
         if (e == cudaSuccess) {
             ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
-            e = launch_coeffs_analytic(dsh, d.n_shapes, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
+            e = launch_coeffs_analytic(dsh, d.n_shapes, dfaces, dedges, c0.x, c0.y, plan->geom.K, N, plan->coef, plan->stream);
         }
         if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
         cudaFree(dsh);
+        if (dfaces) cudaFree(dfaces);
+        if (dedges) cudaFree(dedges);
         CK(e);
         return GSM_OK;
     }
@@ -821,8 +886,16 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
                 return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
     } else {
         for (int i = 0; i < desc->n_shapes; ++i)
-            if (desc->shapes[i].kind != GSM_SPHERE && desc->shapes[i].kind != GSM_ELLIPSOID && desc->shapes[i].kind != GSM_BOX)
+            if (desc->shapes[i].kind < GSM_SPHERE || desc->shapes[i].kind > GSM_POLYHEDRON)
                 return fail(plan, GSM_E_INVALID, "unknown shape kind");
+        for (int i = 0; i < desc->n_shapes; ++i)
+            if (desc->shapes[i].kind == GSM_POLYHEDRON) {
+                ShapeDev q{};
+                std::vector<PolyFace> pf;
+                std::vector<PolyEdge> pe;
+                if (!prepare_polyhedron(desc->shapes[i], q, pf, pe))
+                    return fail(plan, GSM_E_INVALID, "malformed polyhedron (indices, degenerate face, or inward orientation)");
+            }
     }
     // everything that can be rejected has been: from here on the plan's cell is replaced
     plan->desc.eps_bg_re = desc->eps_bg_re; plan->desc.eps_bg_im = desc->eps_bg_im;

@@ -121,10 +121,17 @@ cudaError_t plan_init_attributes();
 struct ShapeDev {
     int kind;
     double c[3], s[3], dre, dim;  // centre, size, (eps_i - eps_bg)/eps_b
-    double f;                     // volume fraction
+    double f;                     // volume fraction (polyhedron: 1 / cell volume, the image carries the volume)
+    int f0, nf;                   // polyhedron: its faces in the PolyFace array
+    double vol;                   // polyhedron: volume
 };
-cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, double c0_re, double c0_im, const double K[3],
-                                   const int N[3], cplx* d_coef, cudaStream_t st);
+// Polyhedron geometry prepared on the host: per face the outward unit normal, the area, one point of the face and its
+// edges; per edge a -> b the midpoint, the half vector (b - a) / 2 and L m (length times in-plane outward normal).
+struct PolyFace { double n[3], p0[3], area; int e0, ne; };
+struct PolyEdge { double mid[3], half[3], mL[3]; };
+cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, const PolyFace* d_faces, const PolyEdge* d_edges,
+                                   double c0_re, double c0_im, const double K[3], const int N[3], cplx* d_coef,
+                                   cudaStream_t st);
 // generic forward FFT along one axis of a dense [outer][P][inner] complex array in global memory (plan time only)
 cudaError_t launch_fft_axis(cplx* d_data, long outer, const AxisPlan& ax, long inner, const cplx* d_tw, cudaStream_t st);
 cudaError_t launch_embed(const cplx* d_coef, const int N[3], const int P[3], cplx* d_pad, cudaStream_t st);

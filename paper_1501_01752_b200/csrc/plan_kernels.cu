@@ -21,7 +21,43 @@ static __device__ double ball_form(double x) {
 }
 static __device__ double sinc_form(double t) { return fabs(t) < 1e-300 ? 1.0 : sin(t) / t; }
 
-__global__ void coeffs_analytic_kernel(const ShapeDev* __restrict__ sh, int nsh, double c0r, double c0i, double K1,
+// int_P exp(-i G.r) d^3r of a polyhedron, divergence theorem twice:
+//   (i / |G|^2) sum_faces (G.n) I_f,  I_f = (i / |G_t|^2) sum_edges (G_t.m) L exp(-i G.mid) sinc(G.half)  or, for G normal
+//   to the face (G_t = 0), I_f = area exp(-i G.p0).  G = 0: the volume.
+static __device__ cplx polyhedron_image(const ShapeDev& q, const PolyFace* __restrict__ faces,
+                                        const PolyEdge* __restrict__ edges, double G1, double G2, double G3) {
+    const double g2 = G1 * G1 + G2 * G2 + G3 * G3;
+    if (g2 == 0.0) return make_double2(q.vol, 0.0);
+    double sr = 0.0, si = 0.0;
+    for (int f = q.f0; f < q.f0 + q.nf; ++f) {
+        const PolyFace F = faces[f];
+        const double Gn = G1 * F.n[0] + G2 * F.n[1] + G3 * F.n[2];
+        const double t1 = G1 - Gn * F.n[0], t2 = G2 - Gn * F.n[1], t3 = G3 - Gn * F.n[2];
+        const double gt2 = t1 * t1 + t2 * t2 + t3 * t3;
+        double ir, ii;
+        if (gt2 < 1e-18 * g2) {
+            double s, c;
+            sincos(-(G1 * F.p0[0] + G2 * F.p0[1] + G3 * F.p0[2]), &s, &c);
+            ir = F.area * c; ii = F.area * s;
+        } else {
+            double ar = 0.0, ai = 0.0;
+            for (int e = F.e0; e < F.e0 + F.ne; ++e) {
+                const PolyEdge E = edges[e];
+                const double x = G1 * E.half[0] + G2 * E.half[1] + G3 * E.half[2];
+                const double w = (t1 * E.mL[0] + t2 * E.mL[1] + t3 * E.mL[2]) * (fabs(x) < 1e-8 ? 1.0 - x * x / 6.0 : sin(x) / x);
+                double s, c;
+                sincos(-(G1 * E.mid[0] + G2 * E.mid[1] + G3 * E.mid[2]), &s, &c);
+                ar += w * c; ai += w * s;
+            }
+            ir = -ai / gt2; ii = ar / gt2;      // times i / |G_t|^2
+        }
+        sr += Gn * ir; si += Gn * ii;
+    }
+    return make_double2(-si / g2, sr / g2);     // times i / |G|^2
+}
+
+__global__ void coeffs_analytic_kernel(const ShapeDev* __restrict__ sh, int nsh, const PolyFace* __restrict__ faces,
+                                       const PolyEdge* __restrict__ edges, double c0r, double c0i, double K1,
                                        double K2, double K3, int N1, int N2, int N3, cplx* __restrict__ coef) {
     const int D1 = 2 * N1 - 1, D2 = 2 * N2 - 1, D3 = 2 * N3 - 1;
     const long total = (long)D1 * D2 * D3;
@@ -32,29 +68,33 @@ __global__ void coeffs_analytic_kernel(const ShapeDev* __restrict__ sh, int nsh,
         if (j1 == N1 - 1 && j2 == N2 - 1 && j3 == N3 - 1) { re = c0r; im = c0i; }
         for (int s = 0; s < nsh; ++s) {
             const ShapeDev q = sh[s];
-            double S;
+            double S, Si = 0.0;
             if (q.kind == GSM_SPHERE) S = ball_form(sqrt(G1 * G1 + G2 * G2 + G3 * G3) * q.s[0]);
             else if (q.kind == GSM_ELLIPSOID) {
                 const double a = G1 * q.s[0], b = G2 * q.s[1], c = G3 * q.s[2];
                 S = ball_form(sqrt(a * a + b * b + c * c));
+            } else if (q.kind == GSM_POLYHEDRON) {
+                const cplx F = polyhedron_image(q, faces, edges, G1, G2, G3);
+                S = F.x; Si = F.y;
             } else S = sinc_form(0.5 * G1 * q.s[0]) * sinc_form(0.5 * G2 * q.s[1]) * sinc_form(0.5 * G3 * q.s[2]);
             double ps, pc;
             sincos(-(G1 * q.c[0] + G2 * q.c[1] + G3 * q.c[2]), &ps, &pc);
-            const double w = q.f * S;
-            // (dre + i dim) * w * (pc + i ps)
-            re += w * (q.dre * pc - q.dim * ps);
-            im += w * (q.dre * ps + q.dim * pc);
+            // (dre + i dim) * f (S + i Si) * (pc + i ps)
+            const double wr = q.f * (S * pc - Si * ps), wi = q.f * (S * ps + Si * pc);
+            re += q.dre * wr - q.dim * wi;
+            im += q.dre * wi + q.dim * wr;
         }
         coef[i] = make_double2(re, im);
     }
 }
 
-cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, double c0_re, double c0_im, const double K[3],
-                                   const int N[3], cplx* d_coef, cudaStream_t st) {
+cudaError_t launch_coeffs_analytic(const ShapeDev* d_shapes, int nshapes, const PolyFace* d_faces, const PolyEdge* d_edges,
+                                   double c0_re, double c0_im, const double K[3], const int N[3], cplx* d_coef,
+                                   cudaStream_t st) {
     const long total = (long)(2 * N[0] - 1) * (2 * N[1] - 1) * (2 * N[2] - 1);
     const int grid = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
-    coeffs_analytic_kernel<<<grid, 256, 0, st>>>(d_shapes, nshapes, c0_re, c0_im, K[0], K[1], K[2], N[0], N[1], N[2],
-                                                 d_coef);
+    coeffs_analytic_kernel<<<grid, 256, 0, st>>>(d_shapes, nshapes, d_faces, d_edges, c0_re, c0_im, K[0], K[1], K[2], N[0],
+                                                 N[1], N[2], d_coef);
     return cudaGetLastError();
 }
 

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgsm_b200.so")
 
 OK, NOT_CONVERGED, E_INVALID, E_ALLOC, E_CUDA, E_SINGULAR_BASIS = 0, 1, -1, -2, -3, -4
-SPHERE, ELLIPSOID, BOX = 0, 1, 2
+SPHERE, ELLIPSOID, BOX, POLYHEDRON = 0, 1, 2, 3
 FORM_E, FORM_H = 0, 1
 FLAG_TWO_SWEEP, FLAG_GENERIC_APPLY, FLAG_FUSED_APPLY = 1, 2, 4   # diagnostics (include/gsm.h GSM_FLAG_*)
 MAX_ITERS = 512
@@ -30,7 +30,9 @@ class GsmError(RuntimeError):
 
 class _Shape(C.Structure):
     _fields_ = [("kind", C.c_int), ("center", C.c_double * 3), ("size", C.c_double * 3),
-                ("eps_re", C.c_double), ("eps_im", C.c_double)]
+                ("eps_re", C.c_double), ("eps_im", C.c_double),
+                ("n_vertices", C.c_int), ("vertices", C.c_void_p), ("n_faces", C.c_int), ("face_sizes", C.c_void_p),
+                ("face_vertices", C.c_void_p)]
 
 
 class _PlanDesc(C.Structure):
@@ -143,16 +145,23 @@ class Plan:
         else:
             shapes = shapes or []
             arr = (_Shape * max(len(shapes), 1))()
+            keep = [arr]
             for i, s in enumerate(shapes):
                 arr[i].kind = int(s["kind"])
                 arr[i].center[:] = [float(v) for v in s["center"]]
                 arr[i].size[:] = [float(v) for v in s["size"]]
                 arr[i].eps_re, arr[i].eps_im = complex(s["eps"]).real, complex(s["eps"]).imag
+                if arr[i].kind == POLYHEDRON:
+                    v = np.ascontiguousarray(s["vertices"], dtype=np.float64).reshape(-1, 3)
+                    fs = np.ascontiguousarray([len(f) for f in s["faces"]], dtype=np.int32)
+                    fv = np.ascontiguousarray([k for f in s["faces"] for k in f], dtype=np.int32)
+                    keep += [v, fs, fv]
+                    arr[i].n_vertices, arr[i].vertices = len(v), v.ctypes.data
+                    arr[i].n_faces, arr[i].face_sizes, arr[i].face_vertices = len(fs), fs.ctypes.data, fv.ctypes.data
             d.n_shapes = len(shapes)
             d.shapes = arr
             d.voxels[:] = [0, 0, 0]
             d.eps_grid_host = None
-            keep = arr
         d.max_iters, d.max_batch = int(max_iters), int(max_batch)
         d.cuda_stream = self.stream.cuda_stream if self.stream is not None else None
         d.formulation = self.formulation

@@ -15,7 +15,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-SPHERE, ELLIPSOID, BOX = 0, 1, 2
+SPHERE, ELLIPSOID, BOX, POLYHEDRON = 0, 1, 2, 3
 TWO_PI = 2.0 * math.pi
 SEED = 150101752
 
@@ -71,6 +71,42 @@ def woodpile(orders=(31, 31, 31), period=0.3, eps_rod=6.25) -> Geometry:
         dict(kind=BOX, center=(L / 2, 0.0, 7 * L / 8), size=(w, L, w), eps=eps_rod),     # y-rod, shifted
     ]
     return _geo("woodpile", (L, L, L), orders, shapes)
+
+
+def polyhedron(name: str, scale: float = 1.0, rotate=None):
+    """Vertices and faces (counter-clockwise seen from outside) of a few convex and one non-convex test polyhedron.
+    rotate = (axis[3], angle): rigid rotation, so that faces are not aligned with the lattice."""
+    if name == "tetrahedron":
+        v = np.array([(1, 1, 1), (1, -1, -1), (-1, 1, -1), (-1, -1, 1)], dtype=float)
+        faces = [(0, 1, 2), (0, 3, 1), (0, 2, 3), (1, 3, 2)]
+    elif name == "cube":
+        v = np.array([(x, y, z) for x in (-1, 1) for y in (-1, 1) for z in (-1, 1)], dtype=float)
+        faces = [(0, 1, 3, 2), (4, 6, 7, 5), (0, 4, 5, 1), (2, 3, 7, 6), (0, 2, 6, 4), (1, 5, 7, 3)]
+    elif name == "octahedron":
+        v = np.array([(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)], dtype=float)
+        faces = [(0, 2, 4), (2, 1, 4), (1, 3, 4), (3, 0, 4), (2, 0, 5), (1, 2, 5), (3, 1, 5), (0, 3, 5)]
+    elif name == "lshape":          # non-convex prism: L-shaped cross-section extruded along z
+        xy = [(-1, -1), (1, -1), (1, 0), (0, 0), (0, 1), (-1, 1)]
+        v = np.array([(x, y, z) for z in (-0.5, 0.5) for (x, y) in xy], dtype=float)
+        faces = [tuple(range(5, -1, -1)), tuple(range(6, 12))] + [(k, (k + 1) % 6, 6 + (k + 1) % 6, 6 + k) for k in range(6)]
+    else:
+        raise ValueError(name)
+    v = v * scale
+    if rotate is not None:
+        ax, ang = np.asarray(rotate[0], dtype=float), float(rotate[1])
+        ax = ax / np.linalg.norm(ax)
+        Kx = np.array([[0, -ax[2], ax[1]], [ax[2], 0, -ax[0]], [-ax[1], ax[0], 0]])
+        R = np.eye(3) + math.sin(ang) * Kx + (1 - math.cos(ang)) * (Kx @ Kx)
+        v = v @ R.T
+    return v, [tuple(int(i) for i in f) for f in faces]
+
+
+def polyhedron_lattice(orders=(7, 7, 7), name="octahedron", period=0.2, scale=0.07, eps=6.0, center=(0.0, 0.0, 0.0),
+                       rotate=((1.0, 2.0, 3.0), 0.4)) -> Geometry:
+    """Cubic lattice of one dielectric polyhedron per cell (analytic Fourier image of a polyhedron)."""
+    v, faces = polyhedron(name, scale, rotate)
+    return _geo(f"poly-{name}", (period,) * 3, orders,
+                [dict(kind=POLYHEDRON, center=center, size=(0, 0, 0), eps=eps, vertices=v, faces=faces)])
 
 
 def random_spheres(seed=SEED, count=20, period=0.25):

@@ -39,6 +39,11 @@ def small_geometries():
         wl.Geometry("mixed-even", (0.2, 0.25, 0.3), (5, 4, 6), off, 1.5, 1.3 + 0.1j, None, ()),
         wl.Geometry("flat", (0.2, 0.25, 0.3), (9, 1, 2), off, 1.0, 1.0, None, ()),
         wl.woodpile((5, 5, 5)),
+        wl.polyhedron_lattice((5, 5, 5), "octahedron", center=(0.02, -0.01, 0.03)),                 # rotated, off-centre
+        wl.polyhedron_lattice((4, 5, 3), "lshape", scale=0.05, rotate=None),                        # non-convex, lattice-aligned faces
+        wl.Geometry("poly-mixed", (0.2, 0.25, 0.3), (5, 4, 6),
+                    off[:1] + wl.polyhedron_lattice((1, 1, 1), "tetrahedron", scale=0.03, eps=7.0 + 0.2j,
+                                                    center=(-0.04, 0.05, -0.06)).shapes, 1.5, 1.3 + 0.1j, None, ()),
     ]
 
 
@@ -49,6 +54,29 @@ def test_coeffs_analytic(geo):
     c_gpu, c_ref = plan.coeffs(), oracle_coeffs(geo)
     assert c_gpu.shape == c_ref.shape
     assert np.max(np.abs(c_gpu - c_ref)) <= 1e-14 * max(1.0, np.max(np.abs(c_ref)))
+    plan.close()
+
+
+def test_polyhedron_rejects_malformed_descriptions_and_solves_vs_dense_lu():
+    """GSM_POLYHEDRON (PAPER.md:62, :99): inward-oriented faces, a bad vertex index and a two-vertex face are rejected;
+    a lattice of rotated cubes is solved against the oracle's dense LU."""
+    geo = wl.polyhedron_lattice((5, 5, 5), "cube", scale=0.05, eps=9.0)
+    sh = geo.shapes[0]
+    for bad in (dict(sh, faces=[tuple(reversed(f)) for f in sh["faces"]]),
+                dict(sh, faces=[(0, 1, 99)] + list(sh["faces"][1:])),
+                dict(sh, faces=[(0, 1)] + list(sh["faces"][1:]))):
+        with pytest.raises(gsm.GsmError) as e:
+            gsm.Plan(geo.periods, geo.orders, shapes=[bad])
+        assert e.value.status == gsm.E_INVALID
+    plan = gsm.plan_from_geometry(geo, max_iters=80)
+    kb, pol = np.array([0.2, -0.1, 1.2 * TWO_PI]), np.array([1.0, 0.3j, 0.0])
+    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    ref = orc.solve_dense(oracle_coeffs(geo), geo.periods, geo.orders, kb, TWO_PI, geo.eps_b, pol)
+    assert st == gsm.OK and resid <= 1e-10 and rel(E.cpu().numpy(), ref) <= 1e-9
+    with pytest.raises(gsm.GsmError):          # set_cell validates before it touches the plan
+        plan.set_cell(geo.periods, shapes=[dict(sh, faces=[(0, 1)] + list(sh["faces"][1:]))])
+    E2, _, _, _, _ = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    assert np.array_equal(E2.cpu().numpy(), E.cpu().numpy())
     plan.close()
 
 

@@ -407,3 +407,65 @@ def test_gmres_with_initial_guess():
     assert m < m0
     E, h, m = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-10, x0=ref)
     assert m == 0 and h == [] and np.array_equal(E, ref)
+
+
+# ---- a0: polyhedron Fourier image -----------------------------------------------------
+def test_polyhedron_image_pinned():
+    """polyhedron_image against things other than itself: (1) an axis-aligned cube is the box closed form (product of
+    sincs) - exercises the G_t = 0 branch; (2) volumes at G = 0 (tetrahedron 8/3 s^3, octahedron 4/3 s^3, L-prism 3 s^3);
+    (3) a rotated tetrahedron against adaptive cubature over its volume (scipy tplquad on the affine image of the unit
+    simplex); (4) a translation multiplies by exp(-i G.t); (5) reversing the face orientation flips the sign;
+    (6) the L-shaped (non-convex) prism equals the difference of two boxes."""
+    v, f = W.polyhedron("cube", 0.03)
+    for G in [(0, 0, 0), (31.4, 0, 0), (31.4, -62.8, 0), (10.0, 20.0, -35.0), (0, 0, 94.2)]:
+        ref = 0.06**3 * np.prod([np.sinc(g * 0.03 / np.pi) for g in G])
+        assert abs(O.polyhedron_image(G, v, f) - ref) < 1e-15 * 0.06**3 * 100
+    s = 0.07
+    assert abs(O.polyhedron_image((0, 0, 0), *W.polyhedron("tetrahedron", s)) - 8 / 3 * s**3) < 1e-18
+    assert abs(O.polyhedron_image((0, 0, 0), *W.polyhedron("octahedron", s)) - 4 / 3 * s**3) < 1e-18
+    assert abs(O.polyhedron_image((0, 0, 0), *W.polyhedron("lshape", s)) - 3 * s**3) < 1e-18
+    v, f = W.polyhedron("tetrahedron", s, rotate=((1.0, 2.0, 3.0), 0.4))
+    M = np.stack([v[1] - v[0], v[2] - v[0], v[3] - v[0]], axis=1)          # r = v0 + M (a, b, c) on the unit simplex
+    jac = abs(np.linalg.det(M))
+    for G in [np.array([31.4, 0.0, 0.0]), np.array([-20.0, 45.0, 12.0])]:
+        def integrand(c, b, a, part):
+            ph = -G @ (v[0] + M @ np.array([a, b, c]))
+            return math.cos(ph) if part == 0 else math.sin(ph)
+        val = [scipy.integrate.tplquad(integrand, 0, 1, lambda a: 0, lambda a: 1 - a, lambda a, b: 0, lambda a, b: 1 - a - b,
+                                       args=(part,), epsabs=1e-13, epsrel=1e-11)[0] for part in (0, 1)]
+        assert abs(O.polyhedron_image(G, v, f) - jac * (val[0] + 1j * val[1])) < 1e-11 * jac
+        t = np.array([0.01, -0.02, 0.015])
+        assert abs(O.polyhedron_image(G, v + t, f) - np.exp(-1j * G @ t) * O.polyhedron_image(G, v, f)) < 1e-18
+        assert abs(O.polyhedron_image(G, v, [tuple(reversed(q)) for q in f]) + O.polyhedron_image(G, v, f)) < 1e-17
+    v, f = W.polyhedron("lshape", s)
+    for G in [(31.4, 0, 0), (10.0, -20.0, 30.0), (0.0, 62.8, 31.4)]:
+        G = np.array(G)
+        big = (2 * s) ** 2 * s * np.prod([np.sinc(g * w / 2 / np.pi) for g, w in zip(G, (2 * s, 2 * s, s))])
+        cut = s * s * s * np.prod([np.sinc(g * s / 2 / np.pi) for g in G]) * np.exp(-1j * (G[0] + G[1]) * s / 2)
+        assert abs(O.polyhedron_image(G, v, f) - (big - cut)) < 1e-16 * 100
+
+
+def test_polyhedron_coefficients_vs_voxelised_direct_dft():
+    """coeffs_analytic with a rotated off-centre octahedron: direct DFT of its voxelisation converges to it; c_0 = f Delta;
+    Hermitian symmetry."""
+    g = W.polyhedron_lattice((3, 3, 3), "octahedron", center=(0.02, -0.01, 0.03))
+    c = coeffs(g)
+    sh = g.shapes[0]
+    L = g.periods[0]
+    assert abs(c[2, 2, 2] - (sh["eps"] - 1.0) * 4 / 3 * 0.07**3 / L**3) < 1e-15
+    assert np.allclose(c, np.conj(c[::-1, ::-1, ::-1]), atol=1e-16)
+    v, faces = sh["vertices"], sh["faces"]
+    normals, offs = [], []
+    for f in faces:                                   # inside <=> n_f.(r - v_f) <= 0 for every face (convex)
+        n = np.cross(v[f[1]] - v[f[0]], v[f[2]] - v[f[0]])
+        normals.append(n / np.linalg.norm(n)); offs.append(normals[-1] @ v[f[0]])
+    errs = []
+    for nv in (16, 48, 96):
+        ax = np.arange(nv) * L / nv
+        r = np.stack(np.meshgrid(ax, ax, ax, indexing="ij"), axis=-1) - np.asarray(sh["center"])
+        r = (r + L / 2) % L - L / 2                   # minimum image
+        inside = np.ones((nv, nv, nv), dtype=bool)
+        for n, o in zip(normals, offs):
+            inside &= (r @ n) <= o
+        errs.append(np.abs(O.coeffs_voxel(np.where(inside, sh["eps"], 1.0), g.orders, 1.0) - c).max())
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 1e-2 * abs(c[2, 2, 2])
