@@ -92,7 +92,7 @@ typedef struct {
  * device FFT of the grid), or 1 when orders[a] == 1. */
 typedef struct {
     double period[3];            /* Lambda_1..3                 */
-    int orders[3];               /* N1..N3 harmonics kept per axis, 1 <= N <= 64                */
+    int orders[3];               /* N1..N3 harmonics kept per axis, 1 <= N <= 256 (Table 1)       */
     double eps_bg_re, eps_bg_im; /* background permittivity of the analytic path                               */
     double eps_b_re, eps_b_im;   /* basis permittivity eps_b; must make every k_m^2 != k_b^2  */
     int n_shapes;

@@ -122,6 +122,99 @@ __global__ void __launch_bounds__(256) xy_conv_kernel(ApplyGeom g, cplx* __restr
     }
 }
 
+// ------------------------------------------------------------------------------ pass 2, split (65..128 harmonics)
+// A 256 x 256 plane pruned to 128 rows is 528 KB: it does not fit one SM.  The plane convolution then runs as three
+// kernels through the global workspace Y[b][c][pos3][i1][pos2] (expanded along y only, 2 |W|):
+//   y_expand   W[i1][i2] --y-FFT (N2 valid in, P2 out)--> Y[i1][pos2]                 rows of i1, YR per CTA
+//   x_conv     Y[.][pos2]: x-FFT (N1 valid in) -> * Chat -> x-IFFT (N1 kept), in place    CB columns of pos2 per CTA
+//   y_contract Y[i1][pos2] --y-IFFT (N2 kept)--> W[i1][i2]
+// Same butterfly network and position order as the single-kernel pass; lanes run along the contiguous index.
+__global__ void __launch_bounds__(256) y_expand_kernel(ApplyGeom g, const cplx* __restrict__ W, const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y / g.ax[2].P, pos3 = blockIdx.y - c * g.ax[2].P;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P2 = g.ax[1].P, N2 = g.N2;
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = tw + P2;                 // T[k2 * YRs + row]
+    const int r0 = blockIdx.x * g.YR, nr = min(g.YR, g.N1 - r0);
+    load_tw(tw, g.tw[1], P2);
+    const long plane = ((long)b * 3 + c) * g.ax[2].P + pos3;
+    const cplx* Wp = W + plane * g.NL + (long)r0 * N2;
+    for (int i = threadIdx.x; i < nr * N2; i += blockDim.x) {
+        const int r = i / N2, i2 = i - r * N2;
+        T[i2 * g.YRs + r] = Wp[i];
+    }
+    __syncthreads();
+    fft_forward(g.ax[1], Lines{T, g.YRs, 1}, nr, tw, N2);
+    cplx* Yp = g.Y + (plane * g.N1 + r0) * P2;
+    for (int i = threadIdx.x; i < nr * P2; i += blockDim.x) {
+        const int r = i / P2, p2 = i - r * P2;
+        Yp[(long)r * P2 + p2] = T[p2 * g.YRs + r];
+    }
+}
+
+__global__ void __launch_bounds__(256) x_conv_kernel(ApplyGeom g, const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y / g.ax[2].P, pos3 = blockIdx.y - c * g.ax[2].P;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P1 = g.ax[0].P, P2 = g.ax[1].P, N1 = g.N1;
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);
+    cplx* B = tw + P1;                 // B[k1 * CBs + col]
+    const int cb0 = blockIdx.x * g.CB, ncol = min(g.CB, P2 - cb0);
+    load_tw(tw, g.tw[0], P1);
+    cplx* Yp = g.Y + (((long)b * 3 + c) * g.ax[2].P + pos3) * N1 * P2 + cb0;
+    for (int i = threadIdx.x; i < N1 * ncol; i += blockDim.x) {
+        const int i1 = i / ncol, col = i - i1 * ncol;
+        B[i1 * g.CBs + col] = Yp[(long)i1 * P2 + col];
+    }
+    __syncthreads();
+    const AxisPlan& ax = g.ax[0];
+    const cplx* chat = g.chat + (long)pos3 * P1 * P2 + cb0;
+    const Lines bb{B, g.CBs, 1};
+    int Ls = P1;
+    for (int s = 0; s + 1 < ax.nst; ++s) {
+        dif_stage_rt(ax.radix[s], bb, bb, ncol, P1, Ls, tw, s == 0 ? N1 : P1);
+        Ls /= ax.radix[s];
+        __syncthreads();
+    }
+    const bool only = ax.nst == 1;
+    mid_stage_rt(ax.radix[ax.nst - 1], bb, bb, ncol, P1, chat, P2, 1, only ? N1 : P1, only ? N1 : P1);
+    __syncthreads();
+    for (int s = ax.nst - 2; s >= 0; --s) {
+        Ls *= ax.radix[s];
+        dit_stage_rt(ax.radix[s], bb, bb, ncol, P1, Ls, tw, s == 0 ? N1 : P1);
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < N1 * ncol; i += blockDim.x) {
+        const int i1 = i / ncol, col = i - i1 * ncol;
+        Yp[(long)i1 * P2 + col] = B[i1 * g.CBs + col];
+    }
+}
+
+__global__ void __launch_bounds__(256) y_contract_kernel(ApplyGeom g, cplx* __restrict__ W, const int* __restrict__ active) {
+    const int b = blockIdx.z, c = blockIdx.y / g.ax[2].P, pos3 = blockIdx.y - c * g.ax[2].P;
+    if (active && !active[b]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P2 = g.ax[1].P, N2 = g.N2;
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = tw + P2;
+    const int r0 = blockIdx.x * g.YR, nr = min(g.YR, g.N1 - r0);
+    load_tw(tw, g.tw[1], P2);
+    const long plane = ((long)b * 3 + c) * g.ax[2].P + pos3;
+    const cplx* Yp = g.Y + (plane * g.N1 + r0) * P2;
+    for (int i = threadIdx.x; i < nr * P2; i += blockDim.x) {
+        const int r = i / P2, p2 = i - r * P2;
+        T[p2 * g.YRs + r] = Yp[(long)r * P2 + p2];
+    }
+    __syncthreads();
+    fft_inverse(g.ax[1], Lines{T, g.YRs, 1}, nr, tw, N2);
+    cplx* Wp = W + plane * g.NL + (long)r0 * N2;
+    for (int i = threadIdx.x; i < nr * N2; i += blockDim.x) {
+        const int r = i / N2, i2 = i - r * N2;
+        Wp[i] = T[i2 * g.YRs + r];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------- pass 3
 __global__ void __launch_bounds__(256) z_inverse_green_kernel(ApplyGeom g, const cplx* __restrict__ W,
                                                               const cplx* __restrict__ x, cplx* __restrict__ y,
@@ -187,10 +280,16 @@ static size_t smem_pass2(const ApplyGeom& g) {
     return sizeof(cplx) * ((size_t)g.ax[0].P + g.ax[1].P + (size_t)g.ax[1].P * g.N1s + (size_t)g.ax[0].P * g.CBs);
 }
 static size_t smem_pass3(const ApplyGeom& g) { return sizeof(cplx) * ((size_t)g.ax[2].P + (size_t)g.ax[2].P * g.RS3); }
+static size_t smem_ypass(const ApplyGeom& g) { return sizeof(cplx) * ((size_t)g.ax[1].P + (size_t)g.ax[1].P * g.YRs); }
+static size_t smem_xpass(const ApplyGeom& g) { return sizeof(cplx) * ((size_t)g.ax[0].P + (size_t)g.ax[0].P * g.CBs); }
 
+size_t apply_smem_plane(const ApplyGeom& g) { return smem_pass2(g); }
 size_t apply_smem_max(const ApplyGeom& g) {
     size_t m = smem_pass1(g);
-    if (smem_pass2(g) > m) m = smem_pass2(g);
+    if (g.split) {
+        if (smem_ypass(g) > m) m = smem_ypass(g);
+        if (smem_xpass(g) > m) m = smem_xpass(g);
+    } else if (smem_pass2(g) > m) m = smem_pass2(g);
     if (smem_pass3(g) > m) m = smem_pass3(g);
     return m;
 }
@@ -204,7 +303,9 @@ void bill_apply(const ApplyGeom& g, bool fused, Profiler* prof, double units) {
         prof->bytes[KC_APPLY_FUSED] += 2.0 * V * units;
     } else {
         prof->bytes[KC_Z_FORWARD] += (V + Wb) * units;
-        prof->bytes[KC_XY_CONV] += 2.0 * Wb * units;
+        // split path: W -> Y, Y in place, Y -> W with |Y| = 3 P3 N1 P2 complex numbers
+        const double Yb = 16.0 * 3.0 * g.ax[2].P * g.N1 * g.ax[1].P;
+        prof->bytes[KC_XY_CONV] += (g.split ? 2.0 * Wb + 4.0 * Yb : 2.0 * Wb) * units;
         prof->bytes[KC_Z_INVERSE_GREEN] += (Wb + 2.0 * V) * units;
     }
 }
@@ -228,7 +329,13 @@ cudaError_t launch_apply(const ApplyGeom& g, int batch, const double* d_kvec, co
     { ProfScope ps_(prof, KC_XY_CONV, st, Cb);
       if (g.chat64) e = launch_xy_conv64(g, batch, d_W, g.chat64, d_active, st);
       else if (g.chat128) e = launch_xy_conv128(g, batch, d_W, g.chat128, d_active, st);
-      else { xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); e = cudaGetLastError(); } }
+      else if (g.split) {
+          const dim3 gy((g.N1 + g.YR - 1) / g.YR, 3 * g.ax[2].P, batch), gx((g.ax[1].P + g.CB - 1) / g.CB, 3 * g.ax[2].P, batch);
+          y_expand_kernel<<<gy, 256, smem_ypass(g), st>>>(g, d_W, d_active);
+          x_conv_kernel<<<gx, 256, smem_xpass(g), st>>>(g, d_active);
+          y_contract_kernel<<<gy, 256, smem_ypass(g), st>>>(g, d_W, d_active);
+          e = cudaGetLastError();
+      } else { xy_conv_kernel<<<dim3(g.ax[2].P, 3, batch), 256, smem_pass2(g), st>>>(g, d_W, d_active); e = cudaGetLastError(); } }
     if (e != cudaSuccess) return e;
     { ProfScope ps_(prof, KC_Z_INVERSE_GREEN, st);
       if (g.chat64) e = launch_z_inverse_green64(g, batch, d_W, d_x, d_y, d_kvec, d_k0, d_active, st);
@@ -243,6 +350,9 @@ cudaError_t apply_init_attributes() {
     cudaError_t e = cudaFuncSetAttribute(z_forward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(xy_conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(z_inverse_green_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(y_expand_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(x_conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(y_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = apply64_init_attributes();
     if (e == cudaSuccess) e = apply128_init_attributes();
     return e;

@@ -318,7 +318,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
     if (out) *out = nullptr;
     if (!desc || !out) return fail(nullptr, GSM_E_INVALID, "null descriptor or output pointer");
     for (int a = 0; a < 3; ++a) {
-        if (desc->orders[a] < 1 || desc->orders[a] > 64) return fail(nullptr, GSM_E_INVALID, "orders must be in [1, 64]");
+        if (desc->orders[a] < 1 || desc->orders[a] > 256) return fail(nullptr, GSM_E_INVALID, "orders must be in [1, 256]");
         if (!(desc->period[a] > 0.0)) return fail(nullptr, GSM_E_INVALID, "periods must be positive");
     }
     if (desc->eps_b_re == 0.0 && desc->eps_b_im == 0.0) return fail(nullptr, GSM_E_INVALID, "eps_b must be non-zero");
@@ -351,12 +351,16 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         if (desc->formulation != GSM_FORM_E && desc->formulation != GSM_FORM_H)
             return fail(plan, GSM_E_INVALID, "formulation must be GSM_FORM_E or GSM_FORM_H");
         g.hform = desc->formulation == GSM_FORM_H;
-        g.L = std::min(g.NL, g.ax[2].P >= 128 ? 16 : 32);
+        g.L = std::min(g.NL, g.ax[2].P >= 512 ? 8 : g.ax[2].P >= 128 ? 16 : 32);
         g.Lst = odd_at_least(g.L);
         g.RS3 = odd_at_least(3 * g.L);
         g.N1s = odd_at_least(g.N1);
         g.CB = std::min(g.ax[1].P, g.ax[0].P >= 128 ? 16 : 32);
         g.CBs = odd_at_least(g.CB);
+        g.YR = std::min(g.N1, g.ax[1].P >= 128 ? 16 : 32);
+        g.YRs = odd_at_least(g.YR);
+        // 65..128 harmonics in x and y: the pruned plane no longer fits one SM's shared memory
+        g.split = apply_smem_plane(g) > 227 * 1024;
         if (apply_smem_max(g) > 227 * 1024) return fail(plan, GSM_E_INVALID, "orders too large for the shared-memory tiles");
         plan->i0 = ((long)(-g.mmin[0]) * N[1] + (-g.mmin[1])) * N[2] + (-g.mmin[2]);
         CK(apply_init_attributes());
@@ -398,6 +402,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         } else {
             CK(dalloc(plan, &plan->W, (size_t)B * 3 * g.ax[2].P * g.NL));
         }
+        if (g.split) CK(dalloc(plan, &g.Y, (size_t)B * 3 * g.ax[2].P * g.N1 * g.ax[1].P));
         CK(dalloc(plan, &plan->xbuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &plan->ybuf, (size_t)B * kd.vlen));
         CK(dalloc(plan, &ks.basis, (size_t)kd.ld * B * kd.vlen));

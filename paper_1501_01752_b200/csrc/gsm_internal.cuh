@@ -50,6 +50,10 @@ struct ApplyGeom {
     int RS3;             // odd row stride (>= 3L) of the pass-3 tile
     int N1s;             // odd row stride (>= N1) of the pass-2 plane
     int CB, CBs;         // columns per x-batch in pass 2 and the odd row stride (>= CB) of its scratch
+    int split;           // 1: the xy plane does not fit shared memory (65..128 harmonics in x and y): pass 2 runs as
+                         // y-expand -> x-convolution -> y-contract through the global workspace Y
+    int YR, YRs;         // rows (i1) per CTA in the y passes of the split path and their odd stride
+    cplx* Y;             // split path: [batch][3][P3][N1][P2], expanded along y only
     const cplx* tw[3];   // device twiddle tables exp(-2 pi i k / P_a)
     const cplx* chat;    // coefficient spectrum, position order, [P3][P1][P2], scaled by 1/(P1 P2 P3)
     const cplx* chat64;  // same, permuted for apply64.cu (null unless apply64_usable)
@@ -96,6 +100,7 @@ cudaError_t apply_fused64_init_attributes(int* grid_out);
 cudaError_t launch_apply_fused64(const ApplyGeom& g, int batch, const double* d_kvec, const double* d_k0, const cplx* d_x,
                                  cplx* d_y, const int* d_active, const Fused64Dev& f, cudaStream_t st);
 size_t apply_smem_max(const ApplyGeom& g);
+size_t apply_smem_plane(const ApplyGeom& g);   // shared memory of the single-kernel xy pass (decides ApplyGeom.split)
 cudaError_t apply_init_attributes();
 // apply128.cu: pass 2 specialised for 128-point x and y axes
 bool apply128_usable(const ApplyGeom& g);

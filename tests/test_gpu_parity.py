@@ -137,6 +137,24 @@ def test_apply_64_point_axes_ragged(orders):
     _apply_case(geo, 2, 13, orc.toeplitz_matvec_c)
 
 
+@pytest.mark.parametrize("orders", [(70, 66, 3), (65, 128, 1), (3, 4, 65), (2, 100, 70), (66, 65, 20)])
+def test_apply_256_point_axes(orders):
+    """65..128 harmonics per axis (256-point transforms): the generic z passes at P3 = 256 and, when both x and y are
+    that long, the split plane pass (y_expand -> x_conv -> y_contract through the global workspace), ragged against
+    every tile size, H-form included for one case."""
+    geo = wl.Geometry("p256", (0.2, 0.25, 0.3), orders, wl.ellipsoid_lattice().shapes, 1.0, 1.1 + 0.05j, None, ())
+    _apply_case(geo, 2, 17, orc.toeplitz_matvec_c)
+    if orders == (70, 66, 3):
+        plan = gsm.plan_from_geometry(geo, max_batch=1, formulation=gsm.FORM_H)
+        D = orc.coeffs_inverse_analytic(geo.periods, geo.orders, geo.shapes, geo.eps_bg, geo.eps_b)
+        x = wl.random_field(1, geo.orders, 3)
+        kb, k0 = np.array([0.3, -0.4, 1.1 * TWO_PI]), 0.9 * TWO_PI
+        y = plan.apply(kb[None], [k0], torch.from_numpy(x).cuda()).cpu().numpy()[0]
+        ref = orc.apply_operator_H(D, x[0], geo.periods, kb, k0, geo.eps_b, orc.toeplitz_matvec_c)
+        assert rel(y, ref) <= 1e-12
+        plan.close()
+
+
 def test_apply_unit_vector_returns_column():
     # x = e_(c, m') -> (T x)_m = c_{m-m'}; with k0 -> G known, check through the oracle's Green multiply
     geo = wl.sphere_lattice((7, 7, 7))
