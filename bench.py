@@ -264,7 +264,36 @@ def run_gsm(args):
     clocks = sampler.stop() if rank == 0 else None
     value = BATCH * world * args.steps / (ms_total * 1e-3)
 
-    # ---- the plain lock-step scan (all points from a zero start), for comparison ----------------------------------------
+    def profiled_pass(levels, nsteps):
+        """nsteps more steps of the same scan with a CUDA event pair around every launch: kernel split and bytes."""
+        plan.profile(True)
+        plan.profile_read(reset=True)
+        barrier()
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        q0.record(stream)
+        for _ in range(nsteps):
+            plan.scan(kb, k0, pol, tol=TOL, levels=levels)
+        q1.record(stream)
+        barrier()
+        pr = plan.profile_read(reset=True)
+        plan.profile(False)
+        return {k: v for k, v in pr.items() if v[0] > 0 and k != "plan"}, q0.elapsed_time(q1) / nsteps
+
+    def kernel_report(timed, nsteps, peak):
+        dom = max(timed, key=lambda k: timed[k][1])
+        n_l, ms_l, by_l = timed[dom]
+        kernels_ms = sum(v[1] for v in timed.values())
+        roof = {"bound": "hbm", "kernel": dom, "achieved": by_l / (ms_l * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": by_l / (ms_l * 1e-3) / 1e9 / peak, "traffic": _traffic(dom, by_l / n_l), "launches": n_l,
+                "avg_launch_ms": ms_l / n_l, "algorithmic_bytes_per_launch": by_l / n_l, "share_of_step": ms_l / kernels_ms}
+        return roof, {k: v[1] / nsteps for k, v in timed.items()}, \
+            {k: (v[2] / (v[1] * 1e-3) / 1e9 if v[1] > 0 and v[2] > 0 else None) for k, v in timed.items()}
+
+    # ---- second pass of the headline scan, profiled: the kernel split and the roofline ------------------------------------
+    timed, ms_profiled = profiled_pass(args.levels, args.steps)
+
+    # ---- the plain lock-step scan (all 256 points in one batch from a zero start): the configuration in which every
+    # launch works on a full batch, i.e. where the kernels themselves are measured against their roofs -----------------
     plan.scan(kb, k0, pol, tol=TOL)
     barrier()
     z0, z1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -274,20 +303,18 @@ def run_gsm(args):
     z1.record(stream)
     barrier()
     z_ms = max_over_ranks(z0.elapsed_time(z1)) / 2
+    z_timed, z_ms_profiled = profiled_pass(None, 2)
 
-    # ---- second pass, same steps, every launch bracketed by CUDA events: the kernel split and the roofline ---------
-    plan.profile(True)
-    plan.profile_read(reset=True)
+    # ---- a longer list through the same plan: 1024 points, max_batch 256 (waves of the mesh scan are chunked) -------------
+    kb4, k04, pol4 = wl.scan_points(wl.kappa_mesh(N_LO, N_HI, 4 * BATCH), 2, 0)
+    plan.scan(kb4, k04, pol4, tol=TOL, levels=args.levels + 2)
     barrier()
-    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    p0.record(stream)
-    for _ in range(args.steps):
-        step()
-    p1.record(stream)
+    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0.record(stream)
+    _, l_iters, l_resid, _ = plan.scan(kb4, k04, pol4, tol=TOL, levels=args.levels + 2)
+    l1.record(stream)
     barrier()
-    ms_profiled = p0.elapsed_time(p1)
-    prof = plan.profile_read(reset=True)
-    plan.profile(False)
+    l_ms = l0.elapsed_time(l1)
 
     # ---- end to end through the C ABI with host buffers ---------------------------------------------------------
     for _ in range(min(args.warmup, 2)):
@@ -373,6 +400,24 @@ def run_gsm(args):
                "note": "working set of one apply (x, y, W, Chat ~ 150 MB) is about the size of L2"}
         p63.close()
         del x63, y63
+        torch.cuda.empty_cache()
+        # ---- the two large sizes of the paper's Table 1 as single solves (context: PAPER.md:111-115 gives 2.2 s and 114 s
+        # on a GTX Titan, the latter with the GMRES basis streamed from host RAM); informational
+        large = []
+        for N in (128, 256):
+            gl = wl.sphere_lattice((N, N, N), period=0.3, radius_frac=0.3, eps=9.0)
+            pl_ = gsm.plan_from_geometry(gl, max_iters=40, max_batch=1, stream=stream)
+            kbl, poll = np.array([0.0, 0.0, 1.3 * TWO_PI]), np.array([1.0, 0, 0], dtype=complex)
+            pl_.solve(kbl, TWO_PI, poll, tol=1e-8)
+            s0.record(stream)
+            _, _, itl, resl, _ = pl_.solve(kbl, TWO_PI, poll, tol=1e-8)
+            s1.record(stream)
+            torch.cuda.synchronize()
+            large.append({"orders": [N, N, N], "unknowns": 3 * N ** 3, "solve_ms": s0.elapsed_time(s1), "iters": int(itl),
+                          "true_resid": float(resl), "device_GB": pl_.info()["device_bytes"] / 1e9})
+            pl_.close()
+            torch.cuda.empty_cache()
+        c5b["large_orders_single_solve"] = large
 
     if world > 1:
         dist.barrier()
@@ -383,11 +428,9 @@ def run_gsm(args):
 
     # ---- roofline of the dominant kernel class -----------------------------------------------------------------
     peak, peak_src = _peaks()
-    timed = {k: v for k, v in prof.items() if v[0] > 0 and k != "plan"}
-    dom = max(timed, key=lambda k: timed[k][1])
-    n_l, ms_l, by_l = timed[dom]
-    achieved = by_l / (ms_l * 1e-3) / 1e9
-    kernels_ms = sum(v[1] for v in timed.values())
+    roof, k_ms, k_gbs = kernel_report(timed, args.steps, peak)
+    roof["peak_source"] = peak_src
+    z_roof, z_k_ms, z_k_gbs = kernel_report(z_timed, 2, peak)
     gpu_launches = int(sum(v[0] for v in timed.values()))
     mean_it = float(np.mean(iters))
     # whole-step figure against SURVEY 8(d)'s B_solve = (m(m+1)/2 + 3m + 1) V + m |Chat| per solve
@@ -397,6 +440,7 @@ def run_gsm(args):
     b_solve = (float(np.sum((iters * (iters + 1.0) / 2 + 3.0 * iters + 1.0) * V)) + 3.0 * V * guessed
                + float(np.sum(iters)) / BATCH * chat_bytes)
     path_gbs = b_solve * args.steps / (ms_total * 1e-3) / 1e9
+    z_b_solve = float(np.sum((z_iters * (z_iters + 1.0) / 2 + 3.0 * z_iters + 1.0) * V)) + float(np.mean(z_iters)) * chat_bytes
 
     # ---- CPU oracle on a bounded sample ---------------------------------------------------------------------------
     cpu_t, cpu_it, cores = oracle_solve_once(geo, kb[0], k0[0], pol[0])
@@ -417,23 +461,30 @@ def run_gsm(args):
                 "includes": "voxel grid H2D from pinned memory + a0 (gsm_plan_set_cell) + gsm_scan + response D2H + host pole search"},
         "gpu_launches": gpu_launches,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": _traffic(dom, by_l / n_l), "peak_source": peak_src,
-                     "launches": n_l, "avg_launch_ms": ms_l / n_l, "algorithmic_bytes_per_launch": by_l / n_l,
-                     "share_of_step": ms_l / kernels_ms},
+        "roofline": roof,
         "path_roofline": {"algorithmic_GBps": path_gbs, "frac": path_gbs / peak,
                           "definition": "SURVEY 8(d) B_solve summed over the batch / step time (profiling off)"},
-        "profiled_pass": {"ms_per_step": ms_profiled / args.steps,
+        "profiled_pass": {"ms_per_step": ms_profiled,
                           "note": "second pass of the same steps with a CUDA event pair around every launch; "
                                   "roofline, kernel_ms_per_step and kernel_GBps come from it, value and e2e do not"},
-        "kernel_ms_per_step": {k: v[1] / args.steps for k, v in timed.items()},
-        "kernel_GBps": {k: (v[2] / (v[1] * 1e-3) / 1e9 if v[1] > 0 and v[2] > 0 else None) for k, v in timed.items()},
+        "kernel_ms_per_step": k_ms,
+        "kernel_GBps": k_gbs,
         "applies_per_s": BATCH * world / (apply_ms * 1e-3),
         "apply": {"ms_per_batch_apply": apply_ms, "algorithmic_GBps": apply_alg_bytes / (apply_ms * 1e-3) / 1e9,
                   "frac": apply_alg_bytes / (apply_ms * 1e-3) / 1e9 / peak, "definition": "(2V x 256 + |Chat|) / time"},
         "lockstep_zero_start": {"value": BATCH * world / (z_ms * 1e-3), "unit": UNIT, "ms_per_step": z_ms,
                                 "mean_iters": float(np.mean(z_iters)), "max_true_resid": float(np.max(z_resid)),
-                                "note": "plain gsm_scan: all 256 points in one lock-step batch from x0 = 0"},
+                                "note": "plain gsm_scan: all 256 points in one lock-step batch from x0 = 0; every launch "
+                                        "works on a full batch, so this is the pass in which the kernels meet their roofs",
+                                "roofline": z_roof,
+                                "path_roofline": {"algorithmic_GBps": z_b_solve / (z_ms * 1e-3) / 1e9,
+                                                  "frac": z_b_solve / (z_ms * 1e-3) / 1e9 / peak},
+                                "profiled_pass_ms_per_step": z_ms_profiled,
+                                "kernel_ms_per_step": z_k_ms, "kernel_GBps": z_k_gbs},
+        "scan_1024_points": {"value": 4 * BATCH / (l_ms * 1e-3), "unit": UNIT, "ms": l_ms,
+                             "ratio_to_256_point_step": l_ms / (ms_total / args.steps),
+                             "mean_iters": float(np.mean(l_iters)), "max_true_resid": float(np.max(l_resid)),
+                             "note": f"same window, 1024 kappa points, max_batch 256, gsm_scan_mesh with {args.levels + 2} waves"},
         "h_form": {"value": BATCH / (h_ms * 1e-3), "unit": UNIT, "ms_per_step": h_ms, "mean_iters": float(np.mean(h_iters)),
                    "max_true_resid": float(np.max(h_resid)), "note": "same workload, Eq. 5 (H-field) formulation, this rank only"},
         "config5b_63cubed": c5b,
