@@ -229,20 +229,30 @@ __global__ void __launch_bounds__(KT) normalize_kernel(KrylovDims d, KrylovState
     }
 }
 
-// y = R^{-1} g (upper triangular, m = iters[b])
-__global__ void backsolve_kernel(KrylovDims d, KrylovState s, int batch) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+// y = R^{-1} g (upper triangular, m = iters[b]).  One warp per solve: the lanes share each row's sum (row i of R is
+// contiguous in k), fixed shuffle tree, so the m dependent steps cost one load round trip each instead of m - i.
+__global__ void __launch_bounds__(128) backsolve_kernel(KrylovDims d, KrylovState s, int batch) {
+    const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (b >= batch) return;
     const int m = s.iters[b];
     const cplx* Rc = s.R + (long)b * d.ld * d.mmax;
     const cplx* g = s.g + (long)b * d.ld;
     cplx* y = s.ycoef + (long)b * d.mmax;
     for (int i = m - 1; i >= 0; --i) {
-        cplx acc = g[i];
-        for (int k = i + 1; k < m; ++k) acc = csub(acc, cmul(Rc[(long)i * d.mmax + k], y[k]));
-        const cplx rii = Rc[(long)i * d.mmax + i];
-        const double inv = 1.0 / (rii.x * rii.x + rii.y * rii.y);
-        y[i] = make_double2((acc.x * rii.x + acc.y * rii.y) * inv, (acc.y * rii.x - acc.x * rii.y) * inv);
+        cplx acc = make_double2(0.0, 0.0);
+        for (int k = i + 1 + lane; k < m; k += 32) acc = cfma(Rc[(long)i * d.mmax + k], y[k], acc);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        }
+        if (lane == 0) {
+            const cplx gi = g[i], rii = Rc[(long)i * d.mmax + i];
+            const double ax = gi.x - acc.x, ay = gi.y - acc.y;
+            const double inv = 1.0 / (rii.x * rii.x + rii.y * rii.y);
+            y[i] = make_double2((ax * rii.x + ay * rii.y) * inv, (ay * rii.x - ax * rii.y) * inv);
+        }
+        __syncwarp();   // y[i] is read by every lane in the next rows
     }
 }
 
@@ -441,7 +451,7 @@ cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batc
 }
 cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
     ProfScope ps_(prof, KC_SMALL, st);
-    backsolve_kernel<<<(batch + 31) / 32, 32, 0, st>>>(d, s, batch);
+    backsolve_kernel<<<(batch + 3) / 4, 128, 0, st>>>(d, s, batch);
     return cudaGetLastError();
 }
 cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st,
