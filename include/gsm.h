@@ -164,7 +164,7 @@ gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const
 /* Scan of an ORDERED mesh: the list is a line in (k, omega) space sampled at equidistant parameter values in list order
  * ("equidistant mesh kappa_p").  The points are solved in `levels` waves, coarse to fine: wave 0 takes
  * every 2^(levels-1)-th point from a zero start, each later wave the points mid-way between those already solved,
- * started from the Lagrange interpolation (up to 4 neighbours) of their solutions (gsm_scan_guess).  Where the
+ * started from the Lagrange interpolation (the 8 nearest solved points) of their solutions (gsm_scan_guess).  Where the
  * responses solved so far show poles inside the mesh (the pole search of Eq. 7-10 in units of the list index), the
  * interpolation is done on the field times prod (t - eta_k), which is smooth across a pole.  Same results as gsm_scan
  * up to the solver tolerance, fewer iterations.  levels = 1 is gsm_scan.  Outputs as gsm_scan, in list order. */

@@ -419,8 +419,8 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &ks.bnorm, (size_t)B));
         CK(dalloc(plan, &ks.guess, (size_t)B));
         CK(dalloc(plan, &plan->d_mesh_idx, (size_t)B));
-        CK(dalloc(plan, &plan->d_mesh_nbr, (size_t)4 * B));
-        CK(dalloc(plan, &plan->d_mesh_wgt, (size_t)4 * B));
+        CK(dalloc(plan, &plan->d_mesh_nbr, (size_t)GSM_MESH_NNB * B));
+        CK(dalloc(plan, &plan->d_mesh_wgt, (size_t)GSM_MESH_NNB * B));
         CK(dalloc(plan, &ks.scale, (size_t)B));
         CK(dalloc(plan, &ks.active, (size_t)B));
         CK(dalloc(plan, &ks.iters, (size_t)B));
@@ -686,8 +686,9 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
         all = plan->mesh_fields;
     }
     const int B = plan->max_batch;
-    std::vector<double> kb(3 * (size_t)B), kk(B), pl(6 * (size_t)B), wgt(8 * (size_t)B), h_resp(6 * (size_t)B), h_resid(B);
-    std::vector<int> idx(B), nbr(4 * (size_t)B), h_iters(B);
+    const int NNB = GSM_MESH_NNB;
+    std::vector<double> kb(3 * (size_t)B), kk(B), pl(6 * (size_t)B), wgt(2 * (size_t)NNB * B), h_resp(6 * (size_t)B), h_resid(B);
+    std::vector<int> idx(B), nbr((size_t)NNB * B), h_iters(B);
     std::vector<double> xi_all(2 * (size_t)npts, 0.0);   // response projected on the amplitude, for the pole estimate
     bool nc = false;
     const int s0 = 1 << (levels - 1);
@@ -700,18 +701,20 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
         // points (multiples of 2 sl: an equidistant mesh) give the poles in units of the list index through the
         // pole search of Eq. 7-10; the guess then interpolates prod_k (t - eta_k) E(t), which is smooth, and divides
         // the product out at the target.  Only the guess changes: the solves and their stop test do not.
-        const int Np = 5, Nd = 10;
-        double pe[2 * Np];
+        const int NpMax = 5;
+        double pe[2 * NpMax];
         int npole = 0;
-        if (lev > 0 && (npts - 1) / (2 * sl) + 1 >= Np + Nd) {
-            const int cnt = (npts - 1) / (2 * sl) + 1;
+        const int cnt0 = lev > 0 ? (npts - 1) / (2 * sl) + 1 : 0;     // solved points so far
+        const int Np = 5, Nd = 10;
+        if (lev > 0 && cnt0 >= Np + Nd) {
+            const int cnt = cnt0;
             std::vector<double> tt(cnt), xs(2 * (size_t)cnt);
             for (int i = 0; i < cnt; ++i) {
                 tt[i] = (double)(2 * sl) * i;
                 xs[2 * i] = xi_all[2 * (size_t)(2 * sl * i)];
                 xs[2 * i + 1] = xi_all[2 * (size_t)(2 * sl * i) + 1];
             }
-            double eta[2 * Np], zeta[2 * Np];
+            double eta[2 * NpMax], zeta[2 * NpMax];
             int best = -1;
             if (gsm_pole_search(cnt, tt.data(), xs.data(), Np, Nd, tt.front(), tt.back(), eta, zeta, &best) == GSM_OK && best >= 0) {
                 const double zmax = std::hypot(zeta[2 * best], zeta[2 * best + 1]);
@@ -734,14 +737,16 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                 kk[nb] = k0[p];
                 for (int q = 0; q < 6; ++q) pl[6 * nb + q] = pol[6 * (size_t)p + q];
                 if (lev > 0) {
-                    int nodes[4], cnt = 0;
-                    const int cand[4] = {p - 3 * sl, p - sl, p + sl, p + 3 * sl};
-                    for (int q = 0; q < 4; ++q)
-                        if (cand[q] >= 0 && cand[q] < npts) nodes[cnt++] = cand[q];
-                    double w[4];
+                    int nodes[GSM_MESH_NNB], cnt = 0;
+                    // nearest solved points first: p -+ s, p -+ 3 s, ...; a missing side is made up from the other one
+                    for (int d = 1; cnt < NNB && d < 4 * NNB; d += 2) {
+                        if (p - d * sl >= 0) nodes[cnt++] = p - d * sl;
+                        if (cnt < NNB && p + d * sl < npts) nodes[cnt++] = p + d * sl;
+                    }
+                    double w[GSM_MESH_NNB];
                     lagrange_weights((double)p, nodes, cnt, w);
-                    for (int q = 0; q < 4; ++q) {
-                        nbr[4 * nb + q] = q < cnt ? nodes[q] : -1;
+                    for (int q = 0; q < NNB; ++q) {
+                        nbr[NNB * nb + q] = q < cnt ? nodes[q] : -1;
                         double wr = q < cnt ? w[q] : 0.0, wi = 0.0;
                         for (int k = 0; k < npole && q < cnt; ++k) {   // times (t_q - eta_k) / (t_p - eta_k)
                             const double ar = nodes[q] - pe[2 * k], ai = -pe[2 * k + 1];
@@ -753,8 +758,8 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                             wr = tr;
                         }
                         if (!std::isfinite(wr) || !std::isfinite(wi)) { wr = q < cnt ? w[q] : 0.0; wi = 0.0; }
-                        wgt[8 * nb + 2 * q] = wr;
-                        wgt[8 * nb + 2 * q + 1] = wi;
+                        wgt[2 * (NNB * nb + q)] = wr;
+                        wgt[2 * (NNB * nb + q) + 1] = wi;
                     }
                 }
             }
@@ -762,8 +767,8 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
             CK(cudaMemcpyAsync(plan->d_mesh_idx, idx.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
             const cplx* x0 = nullptr;
             if (lev > 0) {
-                CK(cudaMemcpyAsync(plan->d_mesh_nbr, nbr.data(), sizeof(int) * 4 * nb, cudaMemcpyHostToDevice, st));
-                CK(cudaMemcpyAsync(plan->d_mesh_wgt, wgt.data(), sizeof(cplx) * 4 * nb, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(plan->d_mesh_nbr, nbr.data(), sizeof(int) * NNB * nb, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(plan->d_mesh_wgt, wgt.data(), sizeof(cplx) * NNB * nb, cudaMemcpyHostToDevice, st));
                 CK(launch_mesh_guess(plan->kd, nb, all, plan->d_mesh_nbr, plan->d_mesh_wgt, plan->xbuf, st, &plan->prof));
                 CK(cudaStreamSynchronize(st));   // the host vectors are rewritten by the next chunk
                 x0 = plan->xbuf;

@@ -184,8 +184,12 @@ cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch,
 cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st,
                                 Profiler* prof);
 // scan over an ordered mesh (gsm_scan_mesh): guesses by interpolation of already solved neighbours, and the scatter
-// of a wave's solutions into the mesh-ordered field array.  nbr[b][4] = neighbour point indices (-1: unused),
-// wgt[b][4] their (complex) weights, idx[b] = point index of solve b.
+// of a wave's solutions into the mesh-ordered field array.  nbr[b][GSM_MESH_NNB] = neighbour point indices (-1: unused),
+// wgt[b][GSM_MESH_NNB] their (complex) weights, idx[b] = point index of solve b.
+#ifndef GSM_MESH_NNB
+#define GSM_MESH_NNB 8   // interpolation nodes per guess: the solved neighbours at distance s, 3 s, 5 s, 7 s on both sides
+                         // (measured on the bench workload, ms per 256-point scan: 4 nodes 30.2, 6 nodes 20.9, 8 nodes 19.0)
+#endif
 cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all, const int* d_nbr, const cplx* d_wgt,
                               cplx* d_x0, cudaStream_t st, Profiler* prof);
 cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,

@@ -375,10 +375,10 @@ __global__ void __launch_bounds__(KT) mesh_guess_kernel(KrylovDims d, const cplx
     cplx acc[E];
 #pragma unroll
     for (int k = 0; k < E; ++k) acc[k] = make_double2(0.0, 0.0);
-    for (int q = 0; q < 4; ++q) {
-        const int p = nbr[4 * b + q];
+    for (int q = 0; q < GSM_MESH_NNB; ++q) {
+        const int p = nbr[GSM_MESH_NNB * b + q];
         if (p < 0) continue;
-        const cplx w = wgt[4 * b + q];
+        const cplx w = wgt[GSM_MESH_NNB * b + q];
 #pragma unroll
         for (int k = 0; k < E; ++k) {
             const long e = e0 + (long)k * KT;

@@ -355,3 +355,41 @@ def test_direction_sweep_off_axis_vs_oracle_goldens():
     with pytest.raises(gsm.GsmError):          # an empty window on any line rejects the call
         plan.retrieve_neff_many(dirs, pols, -1, TWO_PI, [1.02, 1.3, 1.02, 1.02, 1.02], [1.30, 1.2, 1.30, 1.30, 1.30])
     plan.close()
+
+
+def test_scan_mesh_edge_cases_lossy_hform_short_lists():
+    """gsm_scan_mesh where the guess machinery takes its other branches: a lossy inclusion (complex pole, complex
+    interpolation weights), the H-form, lists too short for a pole estimate, more levels than the list supports,
+    max_batch 1 (every wave in chunks of one), a zero-amplitude point inside the mesh.  The fields must equal the
+    plain scan's to the solver tolerance in every case."""
+    k0 = TWO_PI
+    cases = [
+        (wl.sphere_lattice((7, 7, 7), eps=4.0 + 0.3j), gsm.FORM_E, 33, 4, 8),
+        (wl.sphere_lattice((5, 5, 5)), gsm.FORM_H, 40, 3, 16),
+        (wl.sphere_lattice((5, 5, 5)), gsm.FORM_E, 9, 6, 4),          # 9 points: never enough for the pole search
+        (wl.sphere_lattice((5, 5, 5)), gsm.FORM_E, 21, 3, 1),         # one solve at a time
+        (wl.sphere_lattice((5, 5, 5)), gsm.FORM_E, 2, 5, 8),
+    ]
+    for geo, form, npts, levels, mb in cases:
+        kappa = wl.kappa_mesh(1.03, 1.25, npts)
+        kb, kk, pol = wl.scan_points(kappa, 2, 1 if form == gsm.FORM_H else 0)
+        if npts == 21:
+            pol[7] = 0.0                                              # zero source in the middle of the mesh
+        plan = gsm.plan_from_geometry(geo, max_iters=80, max_batch=mb, formulation=form)
+        shape = (npts, 3) + tuple(geo.orders)
+        f1 = torch.empty(shape, dtype=torch.complex128, device="cuda")
+        f2 = torch.empty(shape, dtype=torch.complex128, device="cuda")
+        r1, it1, res1, st1 = plan.scan(kb, kk, pol, tol=1e-12, fields=f1)
+        r2, it2, res2, st2 = plan.scan(kb, kk, pol, tol=1e-12, fields=f2, levels=levels)
+        assert st1 == st2 == gsm.OK and np.all(res2 <= 1e-10), (geo.name, npts)
+        a, b = f1.cpu().numpy(), f2.cpu().numpy()
+        for p in range(npts):
+            nrm = np.linalg.norm(a[p])
+            cond_ok = abs(kappa[p] / k0 - 1.0998) > 0.004 or geo.orders != (7, 7, 7)
+            if nrm == 0.0:
+                assert np.linalg.norm(b[p]) == 0.0 and it2[p] == 0
+            elif cond_ok:
+                assert np.linalg.norm(a[p] - b[p]) <= 1e-9 * nrm, (geo.name, npts, p)
+        if npts >= 33:            # enough solved points for a pole estimate: the guesses pay (shorter lists: any guess is valid)
+            assert it2.sum() < it1.sum()
+        plan.close()
