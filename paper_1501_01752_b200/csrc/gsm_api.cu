@@ -418,6 +418,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &ks.beta, (size_t)B));
         CK(dalloc(plan, &ks.bnorm, (size_t)B));
         CK(dalloc(plan, &ks.guess, (size_t)B));
+        CK(dalloc(plan, &ks.rflag, (size_t)B));
         CK(dalloc(plan, &plan->d_mesh_idx, (size_t)B));
         CK(dalloc(plan, &plan->d_mesh_nbr, (size_t)GSM_MESH_NNB * B));
         CK(dalloc(plan, &plan->d_mesh_wgt, (size_t)GSM_MESH_NNB * B));
@@ -577,8 +578,9 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     }
     CK(launch_backsolve(kd, ks, nb, st, prof));
     CK(launch_combine(kd, ks, nb, d_x0, d_E, st, prof));
-    // true residual with one more apply
-    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, &plan->fused, nullptr, st, prof, (double)nb));
+    // true residual with one more apply; a guess that was accepted without iterating has it already
+    CK(launch_residual_select(kd, ks, nb, st, prof));
+    CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, d_E, plan->ybuf, plan->W, &plan->fused, ks.rflag, st, prof, 0.0));
     CK(launch_true_residual(kd, ks, nb, plan->ybuf, plan->i0, g.n, plan->d_resid, st, prof));
     int* h_iters = reinterpret_cast<int*>(pin + 2);
     double* h_resid = pin + 2 + nb;           // ints occupy at most nb doubles
@@ -587,6 +589,8 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     CK(cudaMemcpyAsync(h_iters, ks.iters, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h_resid, plan->d_resid, sizeof(double) * nb, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h_active, ks.active, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
+    int* h_rflag = reinterpret_cast<int*>(pin + 2 + 9 * (size_t)nb + kd.mmax);
+    CK(cudaMemcpyAsync(h_rflag, ks.rflag, sizeof(int) * nb, cudaMemcpyDeviceToHost, st));
     // E at m = 0: three complex numbers per solve, stride n inside a vector
     CK(cudaMemcpy2DAsync(h_resp, sizeof(cplx), d_E + plan->i0, sizeof(cplx) * g.n, sizeof(cplx), (size_t)3 * nb,
                          cudaMemcpyDeviceToHost, st));
@@ -595,10 +599,10 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
                            cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     {   // bill the iteration loop: solve b ran iterations j = 0 .. m_b - 1, each one apply and one Arnoldi step
-        double s1 = 0.0, s2 = 0.0;   // sum m_b, sum m_b (m_b - 1) / 2
-        for (int b = 0; b < nb; ++b) { const double m = h_iters[b]; s1 += m; s2 += 0.5 * m * (m - 1.0); }
+        double s1 = 0.0, s2 = 0.0, nres = 0.0;   // sum m_b, sum m_b (m_b - 1) / 2, applies of the residual check
+        for (int b = 0; b < nb; ++b) { const double m = h_iters[b]; s1 += m; s2 += 0.5 * m * (m - 1.0); nres += h_rflag[b]; }
         const double V = 16.0 * kd.vlen;
-        bill_apply(g, plan->fused.ring != nullptr, prof, s1);
+        bill_apply(g, plan->fused.ring != nullptr, prof, s1 + nres);
         if (plan->mgs_cs > 0) {
             prof->bytes[KC_ARNOLDI_MGS] += V * (s2 + 3.0 * s1);       // (j + 3) V: w, v_0..v_j, write v_{j+1}
         } else {

@@ -160,6 +160,7 @@ struct KrylovState {   // all device pointers, one entry (or row) per solve of t
     double* beta;      // [batch] ||r0||: norm of the first basis vector's unnormalised form
     double* bnorm;     // [batch] ||b||: the stop test and the reported residuals are relative to it
     int* guess;        // [batch] 1 when the solve starts from an initial guess x0 (r0 = b - A x0, x = x0 + d)
+    int* rflag;        // [batch] 1 when the true residual needs one more apply (0: guess accepted as is, ||r0|| is it)
     double* scale;     // [batch] 1 / h_{j+1,j} of the running iteration
     int* active;       // [batch] 1 while iterating
     int* iters;        // [batch]
@@ -194,7 +195,10 @@ cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all,
                               cplx* d_x0, cudaStream_t st, Profiler* prof);
 cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,
                                 cudaStream_t st, Profiler* prof);
-// resid[b] = || pol delta_m0 - y[b] || / beta[b]
+// rflag[b] = 0 for the solves whose guess met the stop test without iterating (E = x0 and the true residual is the
+// ||r0|| / ||b|| already formed from A x0), 1 for all others
+cudaError_t launch_residual_select(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);
+// resid[b] = || pol delta_m0 - y[b] || / ||b|| where rflag[b] != 0 (y = A E from one more apply), else ||r0|| / ||b||
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
                                  double* d_resid, cudaStream_t st, Profiler* prof);
 cudaError_t krylov_init_attributes();

@@ -296,6 +296,7 @@ template <int E>
 __global__ void __launch_bounds__(KT) resid_part_kernel(KrylovDims d, KrylovState s, int batch, const cplx* __restrict__ y,
                                                         long i0, long n, cplx* __restrict__ r_out) {
     const int b = blockIdx.y;
+    if (!r_out && !s.rflag[b]) return;      // final residual of a solve whose guess was accepted: ||r0|| is known
     __shared__ double wsum[KT / 32];
     const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
     double nn = 0.0;
@@ -324,7 +325,12 @@ __global__ void resid_final_kernel(KrylovDims d, KrylovState s, int batch, doubl
     if (b >= batch) return;
     double nn = 0.0;
     for (int c = 0; c < d.nchunk; ++c) nn += s.part[(long)b * 2 * d.ld * d.nchunk + c].x;
-    resid[b] = s.bnorm[b] > 0.0 ? sqrt(nn) / s.bnorm[b] : 0.0;
+    const double r = s.rflag[b] ? sqrt(nn) : s.beta[b];
+    resid[b] = s.bnorm[b] > 0.0 ? r / s.bnorm[b] : 0.0;
+}
+__global__ void residual_select_kernel(KrylovState s, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) s.rflag[b] = (s.guess[b] && s.iters[b] == 0) ? 0 : 1;
 }
 
 // initial guess, per solve: beta = ||r0|| from the chunk partials; the guess is taken when it beats the zero start
@@ -482,6 +488,11 @@ cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch,
                            Profiler* prof) {
     ProfScope ps_(prof, KC_COMBINE, st);   // (m_b + 1) V per solve, billed by run_batch from the iteration counts
     combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_x0, d_E);
+    return cudaGetLastError();
+}
+cudaError_t launch_residual_select(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
+    residual_select_kernel<<<(batch + 127) / 128, 128, 0, st>>>(s, batch);
     return cudaGetLastError();
 }
 cudaError_t launch_true_residual(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_y, long i0, long n,
