@@ -79,7 +79,8 @@ def _traffic(kernel, alg_bytes_per_launch):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region (B200_PROFILING.md)."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms (B200_PROFILING.md) from the start of the timed region to
+    the end of the profiled second pass (the same steps again): the timed region alone is a few tens of ms."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -89,7 +90,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                          "-lms", "50", "-i", str(self.index)], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -261,7 +262,6 @@ def run_gsm(args):
     e1.record(stream)
     barrier()
     ms_total = max_over_ranks(e0.elapsed_time(e1))
-    clocks = sampler.stop() if rank == 0 else None
     value = BATCH * world * args.steps / (ms_total * 1e-3)
 
     def profiled_pass(levels, nsteps):
@@ -305,6 +305,7 @@ def run_gsm(args):
 
     # ---- second pass of the headline scan, profiled: the kernel split and the roofline ------------------------------------
     timed, ms_profiled = profiled_pass(args.levels, args.steps)
+    clocks = sampler.stop() if rank == 0 else None
 
     # ---- the plain lock-step scan (all 256 points in one batch from a zero start): the configuration in which every
     # launch works on a full batch, i.e. where the kernels themselves are measured against their roofs -----------------
