@@ -88,8 +88,8 @@ typedef struct {
 
 /* Plan descriptor.  Exactly one of (n_shapes > 0, shapes) or (eps_grid_host != NULL) describes the cell.
  * Voxel path: eps_grid_host[voxels[0]][voxels[1]][voxels[2]] complex, sample j at r_a = j_a Lambda_a / voxels[a];
- * each voxels[a] must be a power of two with 2*orders[a]-1 <= voxels[a] <= 512 (the harmonics are taken from a
- * device FFT of the grid), or 1 when orders[a] == 1. */
+ * 2*orders[a]-1 <= voxels[a] <= 2048.  The harmonics are the discrete Fourier transform of the grid: a
+ * device FFT when every voxels[a] is a power of two <= 512, the defining sums (axis by axis) for any other size. */
 typedef struct {
     double period[3];            /* Lambda_1..3                 */
     int orders[3];               /* N1..N3 harmonics kept per axis, 1 <= N <= 256 (Table 1)       */
@@ -170,6 +170,12 @@ gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const
  * up to the solver tolerance, fewer iterations.  levels = 1 is gsm_scan.  Outputs as gsm_scan, in list order. */
 gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
                          double tol, int levels, double* resp_host, int* iters, double* resid, void* d_E_out);
+
+/* Host-only helper (no device work): the solve order and the interpolation stencils gsm_scan_mesh uses for a list of
+ * npts points and `levels` waves.  wave[npts] = wave in which each point is solved (0 = zero start); nodes[npts][8] =
+ * list indices of the points its guess interpolates (-1 = unused; all -1 in wave 0), weights[npts][8] = their Lagrange
+ * weights in the list index (before the pole factor of gsm_scan_mesh). */
+gsm_status gsm_mesh_schedule(int npts, int levels, int* wave, int* nodes, double* weights);
 
 /* Pole search, host side (Eq. 7-10, with xi in the numerator of Eq. 9 - DESIGN.md reading R11).
  * kappa[npts] equidistant and increasing, xi[npts] complex, npts >= Np + Nd.  All npts - Nd sliding windows of

@@ -185,7 +185,14 @@ static bool prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<Poly
     return q.vol > 0.0;
 }
 
-// a0: coefficients c_d on the device, either from closed forms or from an FFT of the voxel grid
+// voxel grid sizes: at least the 2N - 1 harmonics needed per axis (1 is allowed for an axis with one order)
+static bool voxel_dims_ok(const int* V, const int* N) {
+    for (int a = 0; a < 3; ++a)
+        if (V[a] < 2 * N[a] - 1 || V[a] > 2048) return false;
+    return true;
+}
+
+// a0: coefficients c_d on the device, either from closed forms or from a transform of the voxel grid
 static gsm_status build_coeffs(gsm_plan* plan) {
     const gsm_plan_desc& d = plan->desc;
     const int* N = d.orders;
@@ -242,12 +249,26 @@ static gsm_status build_coeffs(gsm_plan* plan) {
         CK(e);
         return GSM_OK;
     }
-    // voxel path: forward FFT of (eps - eps_b)/eps_b on the Nv grid, keep |d_a| <= N_a - 1
+    // voxel path: transform of (eps - eps_b)/eps_b on the Nv grid, keep |d_a| <= N_a - 1
     const int* V = d.voxels;
+    if (!voxel_dims_ok(V, N)) return fail(plan, GSM_E_INVALID, "voxels[a] must satisfy 2N-1 <= voxels <= 2048");
     AxisPlan vax[3];
-    for (int a = 0; a < 3; ++a)
-        if (V[a] < 2 * N[a] - 1 || V[a] > 512 || !make_axis(V[a], V[a], &vax[a]))
-            return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
+    bool pow2 = true;
+    for (int a = 0; a < 3; ++a) pow2 = pow2 && V[a] <= 512 && make_axis(V[a], V[a], &vax[a]);
+    if (!pow2) {   // any other size: the defining sums, axis by axis, each pass keeping only the wanted harmonics
+        const size_t nv = (size_t)V[0] * V[1] * V[2];
+        const size_t n1 = (size_t)V[0] * V[1] * (2 * N[2] - 1), n2 = (size_t)V[0] * (2 * N[1] - 1) * (2 * N[2] - 1);
+        if (!plan->vgrid || plan->vgrid_count != nv + n1 + n2) { CK(dalloc(plan, &plan->vgrid, nv + n1 + n2)); plan->vgrid_count = nv + n1 + n2; }
+        cplx *grid = plan->vgrid, *t1 = grid + nv, *t2 = t1 + n1;
+        cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
+        ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
+        if (e == cudaSuccess) e = launch_voxel_prepare(grid, (long)nv, d.eps_b_re, d.eps_b_im, d.formulation == GSM_FORM_H, plan->stream);
+        if (e == cudaSuccess) e = launch_voxel_dft_axis(grid, (long)V[0] * V[1], V[2], 1, N[2], t1, plan->stream);
+        if (e == cudaSuccess) e = launch_voxel_dft_axis(t1, (long)V[0], V[1], 2 * N[2] - 1, N[1], t2, plan->stream);
+        if (e == cudaSuccess) e = launch_voxel_dft_axis(t2, 1, V[0], (long)(2 * N[1] - 1) * (2 * N[2] - 1), N[0], plan->coef, plan->stream);
+        CK(e);
+        return GSM_OK;
+    }
     if (!plan->vtw[0] || plan->vdim[0] != V[0] || plan->vdim[1] != V[1] || plan->vdim[2] != V[2]) {
         for (int a = 0; a < 3; ++a) {   // twiddles and frequency->position tables of the voxel FFT (kept for re-use)
             CK(upload_twiddles(plan, V[a], &plan->vtw[a]));
@@ -670,13 +691,52 @@ static void lagrange_weights(double t, const int* tn, int cnt, double* w) {
     }
 }
 
+// Wave structure of gsm_scan_mesh (reading R25).  levels is first reduced so that wave 0 holds at least two points.
+static int mesh_levels(int npts, int levels) {
+    while (levels > 1 && (1 << (levels - 1)) >= npts) --levels;
+    return levels;
+}
+// Interpolation stencil of point p in a wave of half-stride sl: the nearest solved points p -+ sl, p -+ 3 sl, ... (up to
+// GSM_MESH_NNB; towards an end of the list the missing side is made up from the other one) and their Lagrange weights.
+static int mesh_stencil(int p, int sl, int npts, int* nodes, double* w) {
+    int cnt = 0;
+    for (int d = 1; cnt < GSM_MESH_NNB && d < 4 * GSM_MESH_NNB; d += 2) {
+        if (p - d * sl >= 0) nodes[cnt++] = p - d * sl;
+        if (cnt < GSM_MESH_NNB && p + d * sl < npts) nodes[cnt++] = p + d * sl;
+    }
+    lagrange_weights((double)p, nodes, cnt, w);
+    return cnt;
+}
+
+extern "C" gsm_status gsm_mesh_schedule(int npts, int levels, int* wave, int* nodes, double* weights) {
+    if (npts < 0 || levels < 1 || levels > 16 || !wave || !nodes || !weights) return GSM_E_INVALID;
+    if (npts == 0) return GSM_OK;
+    levels = mesh_levels(npts, levels);
+    const int s0 = 1 << (levels - 1);
+    for (int lev = 0; lev < levels; ++lev) {
+        const int sl = s0 >> lev;
+        const int first = lev == 0 ? 0 : sl, step = lev == 0 ? s0 : 2 * sl;
+        for (int p = first; p < npts; p += step) {
+            wave[p] = lev;
+            int nd[GSM_MESH_NNB];
+            double w[GSM_MESH_NNB];
+            const int cnt = lev > 0 ? mesh_stencil(p, sl, npts, nd, w) : 0;
+            for (int q = 0; q < GSM_MESH_NNB; ++q) {
+                nodes[(size_t)GSM_MESH_NNB * p + q] = q < cnt ? nd[q] : -1;
+                weights[(size_t)GSM_MESH_NNB * p + q] = q < cnt ? w[q] : 0.0;
+            }
+        }
+    }
+    return GSM_OK;
+}
+
 extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,
                                     double tol, int levels, double* resp_host, int* iters, double* resid, void* d_E_out) {
     if (!plan) return GSM_E_INVALID;
     if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0) || levels < 1 || levels > 16)
         return fail(plan, GSM_E_INVALID, "gsm_scan_mesh: bad argument");
     if (npts == 0) return GSM_OK;
-    while (levels > 1 && (1 << (levels - 1)) >= npts) --levels;
+    levels = mesh_levels(npts, levels);
     const size_t vlen = (size_t)plan->kd.vlen;
     cplx* all = static_cast<cplx*>(d_E_out);
     if (!all) {
@@ -741,14 +801,9 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                 kk[nb] = k0[p];
                 for (int q = 0; q < 6; ++q) pl[6 * nb + q] = pol[6 * (size_t)p + q];
                 if (lev > 0) {
-                    int nodes[GSM_MESH_NNB], cnt = 0;
-                    // nearest solved points first: p -+ s, p -+ 3 s, ...; a missing side is made up from the other one
-                    for (int d = 1; cnt < NNB && d < 4 * NNB; d += 2) {
-                        if (p - d * sl >= 0) nodes[cnt++] = p - d * sl;
-                        if (cnt < NNB && p + d * sl < npts) nodes[cnt++] = p + d * sl;
-                    }
+                    int nodes[GSM_MESH_NNB];
                     double w[GSM_MESH_NNB];
-                    lagrange_weights((double)p, nodes, cnt, w);
+                    const int cnt = mesh_stencil(p, sl, npts, nodes, w);
                     for (int q = 0; q < NNB; ++q) {
                         nbr[NNB * nb + q] = q < cnt ? nodes[q] : -1;
                         double wr = q < cnt ? w[q] : 0.0, wi = 0.0;
@@ -894,10 +949,8 @@ extern "C" gsm_status gsm_plan_set_cell(gsm_plan* plan, const gsm_plan_desc* des
         return fail(plan, GSM_E_INVALID, "shapes missing");
     if (desc->formulation != plan->desc.formulation) return fail(plan, GSM_E_INVALID, "gsm_plan_set_cell: formulation differs");
     if (desc->eps_grid_host) {
-        AxisPlan tmp;
-        for (int a = 0; a < 3; ++a)
-            if (desc->voxels[a] < 2 * desc->orders[a] - 1 || desc->voxels[a] > 512 || !make_axis(desc->voxels[a], desc->voxels[a], &tmp))
-                return fail(plan, GSM_E_INVALID, "voxels[a] must be a power of two with 2N-1 <= voxels <= 512");
+        if (!voxel_dims_ok(desc->voxels, desc->orders))
+            return fail(plan, GSM_E_INVALID, "voxels[a] must satisfy 2N-1 <= voxels <= 2048");
     } else {
         for (int i = 0; i < desc->n_shapes; ++i)
             if (desc->shapes[i].kind < GSM_SPHERE || desc->shapes[i].kind > GSM_POLYHEDRON)

@@ -142,6 +142,8 @@ cudaError_t launch_fft_axis(cplx* d_data, long outer, const AxisPlan& ax, long i
 cudaError_t launch_embed(const cplx* d_coef, const int N[3], const int P[3], cplx* d_pad, cudaStream_t st);
 cudaError_t launch_chat_layout(const cplx* d_padfft, const int P[3], cplx* d_chat, cudaStream_t st);
 cudaError_t launch_voxel_prepare(cplx* d_grid, long count, double epsb_re, double epsb_im, int hform, cudaStream_t st);
+// direct DFT of one axis of [outer][V][inner] keeping |d| <= N - 1: out[outer][2N-1][inner], scaled by 1 / V
+cudaError_t launch_voxel_dft_axis(const cplx* d_in, long outer, int V, long inner, int N, cplx* d_out, cudaStream_t st);
 cudaError_t launch_voxel_extract(const cplx* d_gridfft, const int Nv[3], const int N[3], const int* d_pos1,
                                  const int* d_pos2, const int* d_pos3, cplx* d_coef, cudaStream_t st);
 

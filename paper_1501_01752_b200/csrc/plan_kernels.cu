@@ -206,6 +206,43 @@ cudaError_t launch_voxel_extract(const cplx* d_gridfft, const int Nv[3], const i
     return cudaGetLastError();
 }
 
+// Voxel grids whose sizes are not powers of two: the harmonics |d| <= N - 1 of one axis by the defining sum
+//   out[o][j][i] = (1 / V) sum_k in[o][k][i] exp(-2 pi i d k / V),  d = j - (N - 1),
+// with the phase index (d k) mod V taken in integers and the twiddle from sincospi (exact argument reduction).
+__global__ void __launch_bounds__(256) voxel_dft_axis_kernel(const cplx* __restrict__ in, long outer, int V, long inner,
+                                                             int N, cplx* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tw = reinterpret_cast<cplx*>(smem_raw);   // exp(-2 pi i q / V), q = 0..V-1
+    for (int q = threadIdx.x; q < V; q += blockDim.x) {
+        double s, c;
+        sincospi(-2.0 * (double)q / (double)V, &s, &c);
+        tw[q] = make_double2(c, s);
+    }
+    __syncthreads();
+    const int D = 2 * N - 1;
+    const long total = outer * D * inner;
+    const double sc = 1.0 / (double)V;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < total; i += (long)gridDim.x * blockDim.x) {
+        const long ii = i % inner, j = (i / inner) % D, o = i / (inner * D);
+        const long d = ((j - (N - 1)) % V + V) % V;
+        const cplx* src = in + o * V * inner + ii;
+        cplx acc = make_double2(0.0, 0.0);
+        long q = 0;
+        for (int k = 0; k < V; ++k) {
+            acc = cfma(src[(long)k * inner], tw[q], acc);
+            q += d;
+            if (q >= V) q -= V;
+        }
+        out[i] = make_double2(acc.x * sc, acc.y * sc);
+    }
+}
+cudaError_t launch_voxel_dft_axis(const cplx* d_in, long outer, int V, long inner, int N, cplx* d_out, cudaStream_t st) {
+    const long total = outer * (2 * N - 1) * inner;
+    const int grid = (int)((total + 255) / 256 < 8192 ? (total + 255) / 256 : 8192);
+    voxel_dft_axis_kernel<<<grid, 256, sizeof(cplx) * (size_t)V, st>>>(d_in, outer, V, inner, N, d_out);
+    return cudaGetLastError();
+}
+
 }  // namespace gsm
 
 namespace gsm {

@@ -90,13 +90,24 @@ def test_coeffs_voxel_fft_vs_direct_dft():
     plan.close()
 
 
-def test_coeffs_voxel_rejects_coarse_or_odd_grid():
-    grid = np.ones((8, 8, 8), dtype=np.complex128)
+def test_coeffs_voxel_any_grid_size_and_rejects_coarse_grid():
+    """Voxel grids that are not powers of two go through the defining sums on the device (12 x 9 x 20 for 5 x 3 x 7
+    orders: 9 = 2 N - 1 exactly on one axis), also in the H-form; a grid with fewer than 2 N - 1 samples is rejected."""
+    rng = np.random.default_rng(wl.SEED + 1)
+    grid = (1.0 + 9.0 * rng.random((12, 9, 20))) + 0.3j * rng.random((12, 9, 20))
+    geo = wl.Geometry("vox-odd", (0.2, 0.3, 0.25), (5, 3, 7), [], 1.0, 1.2 + 0.1j, grid, ())
+    plan = gsm.plan_from_geometry(geo)
+    c_gpu, c_ref = plan.coeffs(), oracle_coeffs(geo)
+    assert np.max(np.abs(c_gpu - c_ref)) <= 1e-14 * np.max(np.abs(c_ref))
+    plan.close()
+    plan = gsm.plan_from_geometry(geo, formulation=gsm.FORM_H)
+    D = orc.coeffs_inverse_voxel(grid, geo.orders, geo.eps_b)
+    assert np.max(np.abs(plan.coeffs() - D)) <= 1e-14 * np.max(np.abs(D))
+    plan.close()
+    _apply_case(geo, 2, 21, orc.toeplitz_matvec)
     with pytest.raises(gsm.GsmError) as e:
-        gsm.Plan((1, 1, 1), (7, 7, 7), voxels=grid)
+        gsm.Plan((1, 1, 1), (7, 7, 7), voxels=np.ones((8, 8, 8), dtype=np.complex128))
     assert e.value.status == gsm.E_INVALID
-    with pytest.raises(gsm.GsmError):
-        gsm.Plan((1, 1, 1), (3, 3, 3), voxels=np.ones((12, 12, 12), dtype=np.complex128))
 
 
 # ------------------------------------------------------------------------------------------- a1-a5: operator
@@ -153,6 +164,41 @@ def test_apply_256_point_axes(orders):
         ref = orc.apply_operator_H(D, x[0], geo.periods, kb, k0, geo.eps_b, orc.toeplitz_matvec_c)
         assert rel(y, ref) <= 1e-12
         plan.close()
+
+
+def test_apply_on_a_side_stream_is_ordered_with_the_current_stream():
+    """A plan bound to its own CUDA stream: x is produced on torch's current stream right before the call and y is read on
+    it right after, with no manual synchronisation (Plan.apply orders the two streams both ways)."""
+    geo = wl.sphere_lattice((17, 17, 17))
+    side = torch.cuda.Stream()
+    p_side = gsm.plan_from_geometry(geo, max_batch=4, stream=side)
+    p_ref = gsm.plan_from_geometry(geo, max_batch=4)
+    kb = np.tile(np.array([0.1, -0.2, 1.2 * TWO_PI]), (4, 1)); k0 = np.full(4, TWO_PI)
+    base = torch.from_numpy(wl.random_field(4, geo.orders)).cuda()
+    for rep in range(3):
+        x = base
+        for _ in range(20):                       # a chain of kernels on the current stream that produces x
+            x = x * (1.0 + 1e-3) + 1e-3
+        y = p_side.apply(kb, k0, x)
+        got = y.cpu().numpy()                     # read on the current stream
+        ref = p_ref.apply(kb, k0, x).cpu().numpy()
+        assert np.array_equal(got, ref)
+    p_side.close(); p_ref.close()
+
+
+def test_poles_do_not_depend_on_the_basis_permittivity():
+    """Reading R7 / SURVEY 8(c): multiplying Eq. 4 by (k_m^2 - k_b^2) removes eps_b from the operator, so the poles of the
+    response are the same for every admissible eps_b (only the GMRES iteration count moves).  Config 1, three values."""
+    vals = []
+    for eb in (1.0, 1.7, 0.8 + 0.3j):
+        geo = wl.sphere_lattice((7, 7, 7))
+        geo.eps_b = eb
+        plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=32)
+        n, eps, zeta, st = plan.retrieve_neff([0, 0, 1.0], [1.0, 0, 0], 0, TWO_PI, 1.02, 1.25, tol=1e-12)
+        assert st == gsm.OK
+        vals.append(n)
+        plan.close()
+    assert abs(vals[1] - vals[0]) <= 1e-9 and abs(vals[2] - vals[0]) <= 1e-9
 
 
 def test_apply_unit_vector_returns_column():

@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol(lib_path):
     names = declared_functions()
     assert {"gsm_plan_create", "gsm_plan_destroy", "gsm_apply", "gsm_solve", "gsm_scan", "gsm_pole_search",
             "gsm_plan_set_cell", "gsm_plan_profile", "gsm_plan_profile_read", "gsm_last_error", "gsm_scan_guess",
-            "gsm_scan_mesh", "gsm_retrieve_neff_many"} <= set(names)
+            "gsm_scan_mesh", "gsm_retrieve_neff_many", "gsm_mesh_schedule"} <= set(names)
     lib = ctypes.CDLL(lib_path)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/gsm.h but not exported by {lib_path}"
@@ -60,6 +60,40 @@ def test_binding_has_no_cpu_fallback():
         pytest.skip("a CUDA device is present")
     with pytest.raises(RuntimeError):
         gsm.Plan((1.0, 1.0, 1.0), (3, 3, 3))
+
+
+@pytest.mark.parametrize("npts,levels", [(256, 5), (45, 4), (21, 3), (9, 6), (2, 5), (1, 3), (1024, 7), (100, 1)])
+def test_mesh_schedule_waves_and_stencils(npts, levels):
+    """gsm_mesh_schedule = the host logic of gsm_scan_mesh (reading R25), no device needed: every point is solved exactly
+    once; wave 0 is an equidistant subset holding the first point; a point's interpolation nodes were all solved in
+    EARLIER waves, are distinct, and are the nearest solved points; the Lagrange weights sum to one and reproduce every
+    polynomial of degree below the node count at the point's own index."""
+    from paper_1501_01752_b200 import gsm
+    wave, nodes, w = gsm.mesh_schedule(npts, levels)
+    assert wave.min() == 0 and np.all(wave >= 0)
+    z = np.flatnonzero(wave == 0)
+    assert z[0] == 0 and (len(z) == 1 or len(set(np.diff(z).tolist())) == 1)
+    if npts >= 2:
+        assert len(z) >= 2 or levels == 1 or npts == 2                 # levels were reduced to what the list supports
+    if levels == 1:
+        assert np.all(wave == 0) and np.all(nodes == -1)
+    for p in range(npts):
+        nd = nodes[p][nodes[p] >= 0]
+        if wave[p] == 0:
+            assert len(nd) == 0
+            continue
+        assert len(nd) >= 2 and len(set(nd.tolist())) == len(nd)
+        assert np.all(wave[nd] < wave[p]) and np.all((nd >= 0) & (nd < npts))
+        solved = np.flatnonzero(wave < wave[p])
+        nearest = solved[np.argsort(np.abs(solved - p), kind="stable")[:len(nd)]]
+        assert np.abs(nd - p).max() <= np.abs(nearest - p).max() + 2 * np.abs(nd - p).min()    # a compact neighbourhood
+        wp = w[p][:len(nd)]
+        assert abs(wp.sum() - 1.0) <= 1e-9
+        t = (nd - p) / max(1.0, float(np.abs(nd - p).max()))           # scaled offsets: polynomials in t vanish-order test
+        for deg in range(1, len(nd)):
+            assert abs(np.dot(wp, t**deg)) <= 1e-8 * max(1.0, np.abs(wp).max()), (p, deg)
+    with pytest.raises(gsm.GsmError):
+        gsm.mesh_schedule(5, 0)
 
 
 def test_pole_search_matches_oracle_and_synthetic_poles():
