@@ -164,7 +164,8 @@ gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const
 /* Scan of an ORDERED mesh: the list is a line in (k, omega) space sampled at equidistant parameter values in list order
  * ("equidistant mesh kappa_p").  The points are solved in `levels` waves, coarse to fine: wave 0 takes
  * every 2^(levels-1)-th point from a zero start, each later wave the points mid-way between those already solved,
- * started from the Lagrange interpolation (the 8 nearest solved points) of their solutions (gsm_scan_guess).  Where the
+ * started from the Lagrange interpolation (the 8 nearest solved points) of their solutions (gsm_scan_guess); once a
+ * guessed wave has needed at most one iteration per point on average, all remaining points form the next wave.  Where the
  * responses solved so far show poles inside the mesh (the pole search of Eq. 7-10 in units of the list index), the
  * interpolation is done on the field times prod (t - eta_k), which is smooth across a pole.  Same results as gsm_scan
  * up to the solver tolerance, fewer iterations.  levels = 1 is gsm_scan.  Outputs as gsm_scan, in list order. */
@@ -172,10 +173,11 @@ gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bloch, const 
                          double tol, int levels, double* resp_host, int* iters, double* resid, void* d_E_out);
 
 /* Host-only helper (no device work): the solve order and the interpolation stencils gsm_scan_mesh uses for a list of
- * npts points and `levels` waves.  wave[npts] = wave in which each point is solved (0 = zero start); nodes[npts][8] =
- * list indices of the points its guess interpolates (-1 = unused; all -1 in wave 0), weights[npts][8] = their Lagrange
- * weights in the list index (before the pole factor of gsm_scan_mesh). */
-gsm_status gsm_mesh_schedule(int npts, int levels, int* wave, int* nodes, double* weights);
+ * npts points and `levels` waves.  collapse_after = c > 0: all points still unsolved after wave c form wave c + 1 (what
+ * gsm_scan_mesh does once wave c needed at most one iteration per point); c <= 0: never.  wave[npts] = wave in which each
+ * point is solved (0 = zero start); nodes[npts][8] = list indices of the points its guess interpolates (-1 = unused; all
+ * -1 in wave 0), weights[npts][8] = their Lagrange weights in the list index (before the pole factor of gsm_scan_mesh). */
+gsm_status gsm_mesh_schedule(int npts, int levels, int collapse_after, int* wave, int* nodes, double* weights);
 
 /* Pole search, host side (Eq. 7-10, with xi in the numerator of Eq. 9 - DESIGN.md reading R11).
  * kappa[npts] equidistant and increasing, xi[npts] complex, npts >= Np + Nd.  All npts - Nd sliding windows of

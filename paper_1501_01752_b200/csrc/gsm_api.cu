@@ -696,35 +696,50 @@ static int mesh_levels(int npts, int levels) {
     while (levels > 1 && (1 << (levels - 1)) >= npts) --levels;
     return levels;
 }
-// Interpolation stencil of point p in a wave of half-stride sl: the nearest solved points p -+ sl, p -+ 3 sl, ... (up to
-// GSM_MESH_NNB; towards an end of the list the missing side is made up from the other one) and their Lagrange weights.
-static int mesh_stencil(int p, int sl, int npts, int* nodes, double* w) {
-    int cnt = 0;
-    for (int d = 1; cnt < GSM_MESH_NNB && d < 4 * GSM_MESH_NNB; d += 2) {
-        if (p - d * sl >= 0) nodes[cnt++] = p - d * sl;
-        if (cnt < GSM_MESH_NNB && p + d * sl < npts) nodes[cnt++] = p + d * sl;
+// Interpolation stencil of point p when the multiples of S are solved: the nearest GSM_MESH_NNB of them (towards an end
+// of the list the missing side is made up from the other one) and their Lagrange weights at p.
+static int mesh_stencil(int p, int S, int npts, int* nodes, double* w) {
+    const int last = ((npts - 1) / S) * S;
+    int lo = (p / S) * S, hi = lo + S, cnt = 0;
+    while (cnt < GSM_MESH_NNB && (lo >= 0 || hi <= last)) {
+        const bool take_lo = lo >= 0 && (hi > last || p - lo <= hi - p);
+        if (take_lo) { nodes[cnt++] = lo; lo -= S; } else { nodes[cnt++] = hi; hi += S; }
     }
     lagrange_weights((double)p, nodes, cnt, w);
     return cnt;
 }
+// Points of the next wave when the multiples of S are solved: the odd multiples of S / 2, or - `collapse` - every point
+// that is not solved yet.  Returns the stride of the solved set afterwards.
+static int mesh_wave(int npts, int S, bool collapse, std::vector<int>& targets) {
+    targets.clear();
+    if (collapse) {
+        for (int p = 0; p < npts; ++p)
+            if (p % S) targets.push_back(p);
+        return 1;
+    }
+    for (int p = S / 2; p < npts; p += S) targets.push_back(p);
+    return S / 2;
+}
 
-extern "C" gsm_status gsm_mesh_schedule(int npts, int levels, int* wave, int* nodes, double* weights) {
+extern "C" gsm_status gsm_mesh_schedule(int npts, int levels, int collapse_after, int* wave, int* nodes, double* weights) {
     if (npts < 0 || levels < 1 || levels > 16 || !wave || !nodes || !weights) return GSM_E_INVALID;
     if (npts == 0) return GSM_OK;
     levels = mesh_levels(npts, levels);
-    const int s0 = 1 << (levels - 1);
-    for (int lev = 0; lev < levels; ++lev) {
-        const int sl = s0 >> lev;
-        const int first = lev == 0 ? 0 : sl, step = lev == 0 ? s0 : 2 * sl;
-        for (int p = first; p < npts; p += step) {
-            wave[p] = lev;
+    int S = 1 << (levels - 1);
+    for (int p = 0; p < npts; ++p) {
+        wave[p] = p % S ? -1 : 0;
+        for (int q = 0; q < GSM_MESH_NNB; ++q) { nodes[(size_t)GSM_MESH_NNB * p + q] = -1; weights[(size_t)GSM_MESH_NNB * p + q] = 0.0; }
+    }
+    std::vector<int> targets;
+    for (int w = 1; S > 1; ++w) {
+        const int Sn = S;
+        S = mesh_wave(npts, Sn, collapse_after > 0 && w > collapse_after, targets);
+        for (int p : targets) {
+            wave[p] = w;
             int nd[GSM_MESH_NNB];
-            double w[GSM_MESH_NNB];
-            const int cnt = lev > 0 ? mesh_stencil(p, sl, npts, nd, w) : 0;
-            for (int q = 0; q < GSM_MESH_NNB; ++q) {
-                nodes[(size_t)GSM_MESH_NNB * p + q] = q < cnt ? nd[q] : -1;
-                weights[(size_t)GSM_MESH_NNB * p + q] = q < cnt ? w[q] : 0.0;
-            }
+            double wt[GSM_MESH_NNB];
+            const int cnt = mesh_stencil(p, Sn, npts, nd, wt);
+            for (int q = 0; q < cnt; ++q) { nodes[(size_t)GSM_MESH_NNB * p + q] = nd[q]; weights[(size_t)GSM_MESH_NNB * p + q] = wt[q]; }
         }
     }
     return GSM_OK;
@@ -752,35 +767,37 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
     const int B = plan->max_batch;
     const int NNB = GSM_MESH_NNB;
     std::vector<double> kb(3 * (size_t)B), kk(B), pl(6 * (size_t)B), wgt(2 * (size_t)NNB * B), h_resp(6 * (size_t)B), h_resid(B);
-    std::vector<int> idx(B), nbr((size_t)NNB * B), h_iters(B);
+    std::vector<int> idx(B), nbr((size_t)NNB * B), h_iters(B), targets;
     std::vector<double> xi_all(2 * (size_t)npts, 0.0);   // response projected on the amplitude, for the pole estimate
     bool nc = false;
-    const int s0 = 1 << (levels - 1);
-    for (int lev = 0; lev < levels; ++lev) {
-        // wave 0: multiples of s0 from x0 = 0; wave lev: odd multiples of sl = s0 >> lev, whose neighbours at distance
-        // sl and 3 sl are multiples of 2 sl, i.e. solved by an earlier wave
-        const int sl = s0 >> lev;
+    int S = 1 << (levels - 1);        // the multiples of S are solved (after wave 0)
+    for (int p = 0; p < npts; p += S) targets.push_back(p);
+    double prev_mean = -1.0;          // mean iteration count of the previous guessed wave
+    for (int w = 0; w == 0 || S > 1; ++w) {
+        // Wave 0: the multiples of S from x0 = 0.  Wave w: the points mid-way between the solved ones, guessed from
+        // the nearest solved points - or, once a guessed wave has needed no more than one iteration per point on
+        // average (the guesses are already at the solver tolerance), every remaining point at once.
+        const int Sn = S;             // stride of the solved set the stencils draw from
+        if (w > 0) S = mesh_wave(npts, Sn, prev_mean >= 0.0 && prev_mean <= 1.0, targets);
         // Near a pole eta of the response the field behaves as R / (kappa - eta) + smooth, which
         // polynomial interpolation follows badly - and those are the points that need most iterations.  The solved
-        // points (multiples of 2 sl: an equidistant mesh) give the poles in units of the list index through the
-        // pole search of Eq. 7-10; the guess then interpolates prod_k (t - eta_k) E(t), which is smooth, and divides
-        // the product out at the target.  Only the guess changes: the solves and their stop test do not.
-        const int NpMax = 5;
-        double pe[2 * NpMax];
-        int npole = 0;
-        const int cnt0 = lev > 0 ? (npts - 1) / (2 * sl) + 1 : 0;     // solved points so far
+        // points (multiples of Sn: an equidistant mesh) give the poles in units of the list index through the pole
+        // search of Eq. 7-10; the guess then interpolates prod_k (t - eta_k) E(t), which is smooth, and divides the
+        // product out at the target.  Only the guess changes: the solves and their stop test do not.
         const int Np = 5, Nd = 10;
-        if (lev > 0 && cnt0 >= Np + Nd) {
-            const int cnt = cnt0;
-            std::vector<double> tt(cnt), xs(2 * (size_t)cnt);
-            for (int i = 0; i < cnt; ++i) {
-                tt[i] = (double)(2 * sl) * i;
-                xs[2 * i] = xi_all[2 * (size_t)(2 * sl * i)];
-                xs[2 * i + 1] = xi_all[2 * (size_t)(2 * sl * i) + 1];
+        double pe[2 * Np];
+        int npole = 0;
+        const int cnt0 = w > 0 ? (npts - 1) / Sn + 1 : 0;     // solved points so far
+        if (w > 0 && cnt0 >= Np + Nd) {
+            std::vector<double> tt(cnt0), xs(2 * (size_t)cnt0);
+            for (int i = 0; i < cnt0; ++i) {
+                tt[i] = (double)Sn * i;
+                xs[2 * i] = xi_all[2 * (size_t)Sn * i];
+                xs[2 * i + 1] = xi_all[2 * (size_t)Sn * i + 1];
             }
-            double eta[2 * NpMax], zeta[2 * NpMax];
+            double eta[2 * Np], zeta[2 * Np];
             int best = -1;
-            if (gsm_pole_search(cnt, tt.data(), xs.data(), Np, Nd, tt.front(), tt.back(), eta, zeta, &best) == GSM_OK && best >= 0) {
+            if (gsm_pole_search(cnt0, tt.data(), xs.data(), Np, Nd, tt.front(), tt.back(), eta, zeta, &best) == GSM_OK && best >= 0) {
                 const double zmax = std::hypot(zeta[2 * best], zeta[2 * best + 1]);
                 for (int k = 0; k < Np; ++k)      // every pole inside the mesh whose amplitude matters
                     if (eta[2 * k] >= tt.front() && eta[2 * k] <= tt.back() &&
@@ -791,22 +808,22 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                     }
             }
         }
-        const int first = lev == 0 ? 0 : sl, step = lev == 0 ? s0 : 2 * sl;
-        for (int p0 = first; p0 < npts;) {
-            int nb = 0;
-            for (; nb < B && p0 < npts; ++nb, p0 += step) {
-                const int p = p0;
-                idx[nb] = p;
-                for (int a = 0; a < 3; ++a) kb[3 * nb + a] = k_bloch[3 * (size_t)p + a];
-                kk[nb] = k0[p];
-                for (int q = 0; q < 6; ++q) pl[6 * nb + q] = pol[6 * (size_t)p + q];
-                if (lev > 0) {
+        double wave_iters = 0.0;
+        for (size_t t0 = 0; t0 < targets.size(); t0 += (size_t)B) {
+            const int nb = (int)std::min((size_t)B, targets.size() - t0);
+            for (int b = 0; b < nb; ++b) {
+                const int p = targets[t0 + b];
+                idx[b] = p;
+                for (int a = 0; a < 3; ++a) kb[3 * b + a] = k_bloch[3 * (size_t)p + a];
+                kk[b] = k0[p];
+                for (int q = 0; q < 6; ++q) pl[6 * b + q] = pol[6 * (size_t)p + q];
+                if (w > 0) {
                     int nodes[GSM_MESH_NNB];
-                    double w[GSM_MESH_NNB];
-                    const int cnt = mesh_stencil(p, sl, npts, nodes, w);
+                    double wl[GSM_MESH_NNB];
+                    const int cnt = mesh_stencil(p, Sn, npts, nodes, wl);
                     for (int q = 0; q < NNB; ++q) {
-                        nbr[NNB * nb + q] = q < cnt ? nodes[q] : -1;
-                        double wr = q < cnt ? w[q] : 0.0, wi = 0.0;
+                        nbr[NNB * b + q] = q < cnt ? nodes[q] : -1;
+                        double wr = q < cnt ? wl[q] : 0.0, wi = 0.0;
                         for (int k = 0; k < npole && q < cnt; ++k) {   // times (t_q - eta_k) / (t_p - eta_k)
                             const double ar = nodes[q] - pe[2 * k], ai = -pe[2 * k + 1];
                             const double br = p - pe[2 * k], bi = -pe[2 * k + 1];
@@ -816,25 +833,25 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                             wi = wr * fi + wi * fr;
                             wr = tr;
                         }
-                        if (!std::isfinite(wr) || !std::isfinite(wi)) { wr = q < cnt ? w[q] : 0.0; wi = 0.0; }
-                        wgt[2 * (NNB * nb + q)] = wr;
-                        wgt[2 * (NNB * nb + q) + 1] = wi;
+                        if (!std::isfinite(wr) || !std::isfinite(wi)) { wr = q < cnt ? wl[q] : 0.0; wi = 0.0; }
+                        wgt[2 * (NNB * b + q)] = wr;
+                        wgt[2 * (NNB * b + q) + 1] = wi;
                     }
                 }
             }
             cudaStream_t st = plan->stream;
             CK(cudaMemcpyAsync(plan->d_mesh_idx, idx.data(), sizeof(int) * nb, cudaMemcpyHostToDevice, st));
             const cplx* x0 = nullptr;
-            if (lev > 0) {
+            if (w > 0) {
                 CK(cudaMemcpyAsync(plan->d_mesh_nbr, nbr.data(), sizeof(int) * NNB * nb, cudaMemcpyHostToDevice, st));
                 CK(cudaMemcpyAsync(plan->d_mesh_wgt, wgt.data(), sizeof(cplx) * NNB * nb, cudaMemcpyHostToDevice, st));
                 CK(launch_mesh_guess(plan->kd, nb, all, plan->d_mesh_nbr, plan->d_mesh_wgt, plan->xbuf, st, &plan->prof));
                 CK(cudaStreamSynchronize(st));   // the host vectors are rewritten by the next chunk
                 x0 = plan->xbuf;
             }
-            gsm_status s = run_batch(plan, nb, kb.data(), kk.data(), pl.data(), tol, x0, plan->xbuf, h_resp.data(),
-                                     h_iters.data(), h_resid.data(), nullptr, 0, &nc);
-            if (s != GSM_OK) return s;
+            gsm_status s2 = run_batch(plan, nb, kb.data(), kk.data(), pl.data(), tol, x0, plan->xbuf, h_resp.data(),
+                                      h_iters.data(), h_resid.data(), nullptr, 0, &nc);
+            if (s2 != GSM_OK) return s2;
             CK(launch_mesh_scatter(plan->kd, nb, plan->xbuf, plan->d_mesh_idx, all, st, &plan->prof));
             CK(cudaStreamSynchronize(st));
             for (int b = 0; b < nb; ++b) {
@@ -851,10 +868,12 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
                     xi_all[2 * p] = nrm > 0.0 ? re / nrm : 0.0;
                     xi_all[2 * p + 1] = nrm > 0.0 ? im / nrm : 0.0;
                 }
+                wave_iters += h_iters[b];
                 if (iters) iters[p] = h_iters[b];
                 if (resid) resid[p] = h_resid[b];
             }
         }
+        if (w > 0 && !targets.empty()) prev_mean = wave_iters / (double)targets.size();
     }
     return nc ? GSM_NOT_CONVERGED : GSM_OK;
 }

@@ -62,7 +62,7 @@ def _load():
     lib.gsm_scan.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P]
     lib.gsm_scan_guess.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P, P]
     lib.gsm_scan_mesh.argtypes = [P, C.c_int, P, P, P, C.c_double, C.c_int, P, P, P, P]
-    lib.gsm_mesh_schedule.argtypes = [C.c_int, C.c_int, P, P, P]
+    lib.gsm_mesh_schedule.argtypes = [C.c_int, C.c_int, C.c_int, P, P, P]
     lib.gsm_mesh_schedule.restype = C.c_int
     lib.gsm_pole_search.argtypes = [C.c_int, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P, ip]
     lib.gsm_plan_set_cell.argtypes = [P, C.POINTER(_PlanDesc)]
@@ -310,12 +310,13 @@ class Plan:
         return out[:, 0] + 1j * out[:, 1], out[:, 2] + 1j * out[:, 3], out[:, 4] + 1j * out[:, 5], ls, st
 
 
-def mesh_schedule(npts, levels):
+def mesh_schedule(npts, levels, collapse_after=0):
     """gsm_mesh_schedule (host side): (wave [npts], nodes [npts, 8], weights [npts, 8]) of gsm_scan_mesh."""
     wave = np.full(npts, -1, dtype=np.int32)
     nodes = np.full((npts, 8), -1, dtype=np.int32)
     weights = np.zeros((npts, 8))
-    st = _lib.gsm_mesh_schedule(int(npts), int(levels), wave.ctypes.data, nodes.ctypes.data, weights.ctypes.data)
+    st = _lib.gsm_mesh_schedule(int(npts), int(levels), int(collapse_after), wave.ctypes.data, nodes.ctypes.data,
+                                weights.ctypes.data)
     if st < 0:
         raise GsmError(st, "gsm_mesh_schedule: invalid arguments")
     return wave, nodes, weights

@@ -62,15 +62,18 @@ def test_binding_has_no_cpu_fallback():
         gsm.Plan((1.0, 1.0, 1.0), (3, 3, 3))
 
 
-@pytest.mark.parametrize("npts,levels", [(256, 5), (45, 4), (21, 3), (9, 6), (2, 5), (1, 3), (1024, 7), (100, 1)])
-def test_mesh_schedule_waves_and_stencils(npts, levels):
+@pytest.mark.parametrize("npts,levels,collapse", [(256, 5, 0), (256, 5, 1), (45, 4, 2), (45, 4, 0), (21, 3, 0), (9, 6, 1),
+                                                  (2, 5, 0), (1, 3, 0), (1024, 7, 1), (100, 1, 0)])
+def test_mesh_schedule_waves_and_stencils(npts, levels, collapse):
     """gsm_mesh_schedule = the host logic of gsm_scan_mesh (reading R25), no device needed: every point is solved exactly
     once; wave 0 is an equidistant subset holding the first point; a point's interpolation nodes were all solved in
     EARLIER waves, are distinct, and are the nearest solved points; the Lagrange weights sum to one and reproduce every
     polynomial of degree below the node count at the point's own index."""
     from paper_1501_01752_b200 import gsm
-    wave, nodes, w = gsm.mesh_schedule(npts, levels)
+    wave, nodes, w = gsm.mesh_schedule(npts, levels, collapse)
     assert wave.min() == 0 and np.all(wave >= 0)
+    if collapse > 0:
+        assert wave.max() <= collapse + 1
     z = np.flatnonzero(wave == 0)
     assert z[0] == 0 and (len(z) == 1 or len(set(np.diff(z).tolist())) == 1)
     if npts >= 2:
