@@ -342,7 +342,13 @@ def run_gsm(args):
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e_value = BATCH * world * args.steps / e2e_s
     h2d = int(pinned_grid.numel() * 16 + kb.nbytes + k0.nbytes + pol.nbytes + 16)
-    d2h = int(resp.nbytes + iters.nbytes + resid.nbytes + 4 * BATCH + 4 * int(np.max(iters)))   # + active flags, nactive per iteration
+    # per solve: response (48 B), iterations, residual, active flag, residual-check flag; per lock-step tick: nactive (4 B)
+    if args.levels > 1:
+        wave_of, _, _ = gsm.mesh_schedule(BATCH, args.levels, 1)
+        ticks = sum(int(iters[wave_of == w].max()) + 2 for w in range(int(wave_of.max()) + 1))
+    else:
+        ticks = int(np.max(iters)) + 2
+    d2h = int(resp.nbytes + iters.nbytes + resid.nbytes + 8 * BATCH + 4 * ticks)
 
     # ---- operator applies/s (the other half of BASELINE.json's metric) -------------------------------------------
     x = torch.randn((BATCH, 3) + ORDERS, dtype=torch.complex128, device="cuda")
