@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(256) z_forward_kernel(ApplyGeom g, const cplx*
     const int l0 = blockIdx.x * g.L;
     const int nl = min(g.L, g.NL - l0);
     load_tw(tw, g.tw[2], P3);
+    x += slot_offset(g, b);
     const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l0 * N3;
     if (!g.hform) {
         for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
@@ -242,7 +243,7 @@ __global__ void __launch_bounds__(256) z_inverse_green_kernel(ApplyGeom g, const
     // Green dyadic: k_m = k_inc + m o K, k_b^2 = k0^2 eps_b, unconjugated k.k
     const double kx0 = kvec[3 * b + 0], ky0 = kvec[3 * b + 1], kz0 = kvec[3 * b + 2], k0 = k0s[b];
     const double kb2r = k0 * k0 * g.epsb_re, kb2i = k0 * k0 * g.epsb_im;
-    const long base = (long)b * 3 * g.n + (long)l0 * N3;
+    const long base = (long)b * 3 * g.n + (long)l0 * N3 + slot_offset(g, b);
     for (int i = threadIdx.x; i < nl * N3; i += blockDim.x) {
         const int l = i / N3, i3 = i - l * N3;
         const int lg = l0 + l, i1 = lg / g.N2, i2 = lg - i1 * g.N2;

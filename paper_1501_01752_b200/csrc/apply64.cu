@@ -131,6 +131,7 @@ __global__ void __launch_bounds__(256, ZF64_MINB) z_forward64_kernel(ApplyGeom g
     load_group_twiddles(tw, g.tw[2], u);
     cplx* sc = scratch + (warp * 4 + ln) * SC_LINE;
     const int l0 = blockIdx.x * 32, line = warp * 4 + ln, l = l0 + line;
+    x += slot_offset(g, b);
     const cplx* xs = x + ((long)b * 3 + c) * g.n + (long)l * N3;
     cplx a[8];
     if (!HFORM) {
@@ -238,7 +239,7 @@ __global__ void __launch_bounds__(256, 2) z_inverse_green64_kernel(ApplyGeom g, 
     const double k1 = kvec[3 * b + 0] + (i1 + g.mmin[0]) * g.K[0];
     const double k2 = kvec[3 * b + 1] + (i2 + g.mmin[1]) * g.K[1];
     const double k12 = k1 * k1 + k2 * k2;
-    const long base = (long)b * 3 * g.n + (long)l * N3;
+    const long base = (long)b * 3 * g.n + (long)l * N3 + slot_offset(g, b);
 #pragma unroll
     for (int p = 0; p < 4; ++p) {
         const int i3 = u + 8 * p;

@@ -25,7 +25,8 @@ namespace cg = cooperative_groups;
 namespace gsm {
 
 #define MGS_T 256        // threads per CTA
-#define MGS_E 22         // complex elements of w per thread (registers)
+#define MGS_E_LO 22      // complex elements of w per thread (registers): the kernel is instantiated for 22 (31^3: 5586 per
+#define MGS_E_HI 24      // CTA) and 24 (32^3: 6144 per CTA, the most two slice buffers of a CTA leave room for)
 #define MGS_MAXCS 16     // largest cluster (non-portable size, opt-in)
 #define MGS_NW (MGS_T / 32)
 
@@ -115,6 +116,7 @@ static __device__ __forceinline__ cplx cluster_sum_recv(MgsSmem* sm, int step, u
 // chunk = elements per CTA (<= MGS_T * MGS_E).  The first two basis slices of the NEXT solve are requested as soon as
 // the last slice of the current one has been used, so the norm exchange, the write of v_{j+1}, the Givens update and
 // the load of the next w all run under that transfer.
+template <int MGS_E>
 __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, KrylovState s, int batch, int j, int chunk) {
     cg::cluster_group cluster = cg::this_cluster();
     const unsigned cs = cluster.num_blocks(), rank = cluster.block_rank();
@@ -147,11 +149,13 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
         while (from < batch && !s.active[from]) from += nclusters;
         return from;
     };
+    // j < 0: slot-refill scan, every solve is at its own Arnoldi index s.iters[b] (only this cluster changes it)
+    auto index_of = [&](int bb) { return j >= 0 ? j : s.iters[bb]; };
     auto prefetch_first_two = [&](int bb) {   // thread 0 only
         const cplx* vb = s.basis + (long)bb * d.vlen + lo;
         mbar_expect_tx(&sm->mbar[0], bytes);
         bulk_g2s(vbuf0, vb, bytes, &sm->mbar[0]);
-        if (j >= 1) {
+        if (index_of(bb) >= 1) {
             mbar_expect_tx(&sm->mbar[1], bytes);
             bulk_g2s(vbuf1, vb + vs, bytes, &sm->mbar[1]);
         }
@@ -164,6 +168,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     uint32_t phase0 = 0, phase1 = 0;
     int xstep = 0;   // running exchange number of cluster_sum
     while (b < batch) {
+        const int j = index_of(b);                                   // this solve's Arnoldi index
         const cplx* vb = s.basis + (long)b * d.vlen + lo;            // slice of v_0; v_i at + i * vs
         cplx* wg = s.basis + (long)b * d.vlen + (long)(j + 1) * vs + lo;
         if (rank == 0)
@@ -230,6 +235,11 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     cluster.sync();   // no CTA leaves while a peer's asynchronous store to it could still be in flight
 }
 
+// the instantiation whose per-thread registers hold a CTA's slice of w
+static const void* mgs_kernel_for(int chunk) {
+    return chunk <= MGS_T * MGS_E_LO ? (const void*)arnoldi_mgs_kernel<MGS_E_LO> : (const void*)arnoldi_mgs_kernel<MGS_E_HI>;
+}
+
 size_t arnoldi_cluster_smem(const KrylovDims& d, int chunk) {
     return sizeof(cplx) * (2 * (size_t)chunk + d.ld + d.mmax) + sizeof(double) * (d.mmax + (d.mmax & 1)) +
            sizeof(MgsSmem) + 128;
@@ -241,7 +251,7 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     *nclusters_out = 0;
     *cs_out = 0;
     *chunk_out = 0;
-    const long cap = (long)MGS_T * MGS_E;
+    const long cap = (long)MGS_T * MGS_E_HI;
     int cs = 1;
     while (cs <= MGS_MAXCS && (d.vlen + cs - 1) / cs > cap) cs *= 2;
     if (cs > MGS_MAXCS) return cudaSuccess;
@@ -250,10 +260,11 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     if (smem > 227 * 1024) return cudaSuccess;
     // the attribute is per function, not per plan: always ask for the device maximum so that plans of different
     // sizes can coexist
-    cudaError_t e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    const void* kern = mgs_kernel_for(chunk);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     if (cs > 8) {
-        e = cudaFuncSetAttribute(arnoldi_mgs_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (e != cudaSuccess) { cudaGetLastError(); return cudaSuccess; }
     }
     cudaLaunchConfig_t cfg = {};
@@ -268,7 +279,7 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     cfg.attrs = at;
     cfg.numAttrs = 1;
     int nclusters = 0;
-    e = cudaOccupancyMaxActiveClusters(&nclusters, arnoldi_mgs_kernel, &cfg);
+    e = cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg);
     if (e != cudaSuccess || nclusters < 1) { cudaGetLastError(); return cudaSuccess; }
     *cs_out = cs;
     *chunk_out = chunk;
@@ -291,7 +302,8 @@ cudaError_t launch_arnoldi_cluster(const KrylovDims& d, const KrylovState& s, in
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, arnoldi_mgs_kernel, d, s, batch, j, chunk);
+    void* args[] = {(void*)&d, (void*)&s, (void*)&batch, (void*)&j, (void*)&chunk};
+    return cudaLaunchKernelExC(&cfg, mgs_kernel_for(chunk), args);
 }
 
 }  // namespace gsm

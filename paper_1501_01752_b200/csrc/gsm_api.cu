@@ -40,6 +40,9 @@ struct gsm_plan {
     size_t mesh_cap = 0;
     int *d_mesh_idx = nullptr, *d_mesh_nbr = nullptr;   // [max_batch], [max_batch][4]
     cplx* d_mesh_wgt = nullptr;                         // [max_batch][4]
+    void* refill_buf = nullptr;   // slot-refill scan: point list and per-point outputs on the device (grown on demand)
+    size_t refill_cap = 0;        // points it holds
+    int* d_refill_ctl = nullptr;  // [2] next point, points done
     void* pinned = nullptr;       // host staging: nactive, iters, resid, hist
     size_t pinned_bytes = 0;
     mutable std::string err;
@@ -440,6 +443,11 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &ks.bnorm, (size_t)B));
         CK(dalloc(plan, &ks.guess, (size_t)B));
         CK(dalloc(plan, &ks.rflag, (size_t)B));
+        CK(dalloc(plan, &ks.running, (size_t)B));
+        CK(dalloc(plan, &ks.fin, (size_t)B));
+        CK(dalloc(plan, &ks.point, (size_t)B));
+        CK(dalloc(plan, &ks.newv, (size_t)B));
+        CK(dalloc(plan, &plan->d_refill_ctl, (size_t)2));
         CK(dalloc(plan, &plan->d_mesh_idx, (size_t)B));
         CK(dalloc(plan, &plan->d_mesh_nbr, (size_t)GSM_MESH_NNB * B));
         CK(dalloc(plan, &plan->d_mesh_wgt, (size_t)GSM_MESH_NNB * B));
@@ -475,6 +483,7 @@ extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
     for (cudaEvent_t e : plan->iter_ev) if (e) cudaEventDestroy(e);
     for (void* p : plan->allocs) cudaFree(p);
     if (plan->mesh_fields) cudaFree(plan->mesh_fields);
+    if (plan->refill_buf) cudaFree(plan->refill_buf);
     if (plan->pinned) cudaFreeHost(plan->pinned);
     delete plan;
     return GSM_OK;
@@ -646,6 +655,93 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     return GSM_OK;
 }
 
+// Slot-refill scan from a zero start (npts > max_batch, cluster Gram-Schmidt path): max_batch slots run in lock step, each
+// at its own Arnoldi index; a slot whose solve has finished (true residual checked with one more apply, results recorded
+// under its point index) takes the next pending point at the next tick.  Per solve the arithmetic is that of run_batch.
+static gsm_status run_refill(gsm_plan* plan, int npts, const double* kvec, const double* k0, const double* pol, double tol,
+                             cplx* d_E_out, double* resp, int* iters, double* resid, bool* not_converged) {
+    const KrylovDims& kd = plan->kd;
+    const KrylovState& ks = plan->ks;
+    cudaStream_t st = plan->stream;
+    Profiler* prof = &plan->prof;
+    const int B = plan->max_batch;
+    if (singular_basis(plan, npts, kvec, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
+    // device copy of the list and per-point outputs: [resp 6][kvec 3][k0 1][pol 6][resid 1] doubles, [iters][flag] ints
+    const size_t per_pt = sizeof(double) * 17 + sizeof(int) * 2;
+    if (plan->refill_cap < (size_t)npts) {
+        if (plan->refill_buf) cudaFree(plan->refill_buf);
+        plan->refill_buf = nullptr;
+        plan->refill_cap = 0;
+        CK(cudaMalloc(&plan->refill_buf, per_pt * (size_t)npts));
+        plan->refill_cap = (size_t)npts;
+    }
+    double* dd = static_cast<double*>(plan->refill_buf);
+    cplx* d_resp = reinterpret_cast<cplx*>(dd);   // first: 16-byte aligned for any npts
+    double *d_kv = dd + 6 * (size_t)npts, *d_k0 = dd + 9 * (size_t)npts, *d_pol = dd + 10 * (size_t)npts, *d_res = dd + 16 * (size_t)npts;
+    int* d_it = reinterpret_cast<int*>(dd + 17 * (size_t)npts);
+    int* d_flag = d_it + npts;
+    CK(cudaMemcpyAsync(d_kv, kvec, sizeof(double) * 3 * npts, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_k0, k0, sizeof(double) * npts, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_pol, pol, sizeof(double) * 6 * npts, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ks.tol, &tol, sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(ks.nactive, 0, sizeof(int), st));
+    CK(cudaMemsetAsync(plan->d_refill_ctl, 0, 2 * sizeof(int), st));
+    for (int* flags : {ks.running, ks.fin, ks.active, ks.newv, ks.rflag}) CK(cudaMemsetAsync(flags, 0, sizeof(int) * B, st));
+    RefillDev r{d_kv, d_k0, d_pol, npts, plan->d_refill_ctl, plan->d_refill_ctl + 1, d_it, d_res, d_resp, d_flag};
+    ApplyGeom gs = plan->geom;            // the Arnoldi applies: x = v_{j_b}, y = slot j_b + 1 of the basis pool
+    gs.jslot = ks.iters;
+    gs.jstride = (long)B * kd.vlen;
+    const size_t vs = (size_t)B * kd.vlen;
+    int* pin_i = static_cast<int*>(plan->pinned);
+    // first fill: every slot is free
+    CK(launch_refill_commit(kd, ks, r, B, plan->i0, plan->geom.n, plan->xbuf, plan->d_resid, plan->d_kvec, plan->d_k0, st, prof));
+    const long max_ticks = ((long)npts / B + 2) * ((long)kd.mmax + 2);
+    for (long t = 0; t < max_ticks; ++t) {
+        CK(launch_apply(gs, B, plan->d_kvec, plan->d_k0, ks.basis, ks.basis + vs, plan->W, &plan->fused, ks.active, st, prof, 0.0));
+        CK(launch_arnoldi_cluster(kd, ks, B, -1, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, st, prof));
+        // solves that finished in this tick: x = sum y_i v_i, true residual with one more apply, results recorded, slot refilled
+        CK(launch_refill_mark(kd, ks, B, st, prof));
+        CK(launch_backsolve(kd, ks, B, st, prof, ks.fin));
+        CK(launch_combine(kd, ks, B, nullptr, plan->xbuf, st, prof, ks.fin));
+        CK(launch_apply(plan->geom, B, plan->d_kvec, plan->d_k0, plan->xbuf, plan->ybuf, plan->W, &plan->fused, ks.rflag, st, prof, 0.0));
+        CK(launch_true_residual(kd, ks, B, plan->ybuf, plan->i0, plan->geom.n, plan->d_resid, st, prof));
+        if (d_E_out) CK(launch_mesh_scatter(kd, B, plan->xbuf, ks.point, d_E_out, st, prof, ks.fin));
+        CK(launch_refill_commit(kd, ks, r, B, plan->i0, plan->geom.n, plan->xbuf, plan->d_resid, plan->d_kvec, plan->d_k0, st, prof));
+        // the count of recorded points comes back one tick late, so that no launch waits for a round trip
+        CK(cudaMemcpyAsync(pin_i + (t & 1), r.ndone, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(plan->iter_ev[t & 1], st));
+        if (t >= 1) {
+            CK(cudaEventSynchronize(plan->iter_ev[(t - 1) & 1]));
+            if (pin_i[(t - 1) & 1] >= npts) break;
+        }
+    }
+    std::vector<int> h_it(npts), h_flag(npts);
+    std::vector<double> h_res(npts), h_resp(6 * (size_t)npts);
+    CK(cudaMemcpyAsync(h_it.data(), d_it, sizeof(int) * npts, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_flag.data(), d_flag, sizeof(int) * npts, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_res.data(), d_res, sizeof(double) * npts, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_resp.data(), d_resp, sizeof(cplx) * 3 * npts, cudaMemcpyDeviceToHost, st));
+    int done = 0;
+    CK(cudaMemcpyAsync(&done, r.ndone, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (done < npts) return fail(plan, GSM_E_CUDA, "slot-refill scan ended before every point was solved");
+    double s1 = 0.0, s2 = 0.0;
+    for (int p = 0; p < npts; ++p) {
+        const double m = h_it[p];
+        s1 += m;
+        s2 += 0.5 * m * (m - 1.0);
+        if (iters) iters[p] = h_it[p];
+        if (resid) resid[p] = h_res[p];
+        if (h_flag[p]) *not_converged = true;
+        if (resp) for (int q = 0; q < 6; ++q) resp[6 * (size_t)p + q] = h_resp[6 * (size_t)p + q];
+    }
+    const double V = 16.0 * kd.vlen;
+    bill_apply(plan->geom, false, prof, s1 + npts);
+    prof->bytes[KC_ARNOLDI_MGS] += V * (s2 + 3.0 * s1);
+    prof->bytes[KC_COMBINE] += V * (s1 + npts);
+    return GSM_OK;
+}
+
 extern "C" gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double k0, const double pol[6], double tol,
                                 void* d_E_out, double* resid_hist_host, int hist_cap, int* n_iters,
                                 double* true_rel_resid) {
@@ -664,6 +760,11 @@ extern "C" gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_b
     if (!plan) return GSM_E_INVALID;
     if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_scan: bad argument");
     bool nc = false;
+    if (!d_x0 && npts > plan->max_batch && plan->mgs_cs > 0 && !plan->fused.ring) {   // keep the lock-step batch full
+        gsm_status s = run_refill(plan, npts, k_bloch, k0, pol, tol, static_cast<cplx*>(d_E_out), resp_host, iters, resid, &nc);
+        if (s != GSM_OK) return s;
+        return nc ? GSM_NOT_CONVERGED : GSM_OK;
+    }
     for (int p0 = 0; p0 < npts; p0 += plan->max_batch) {
         const int nb = std::min(plan->max_batch, npts - p0);
         cplx* dE = d_E_out ? static_cast<cplx*>(d_E_out) + (size_t)p0 * plan->kd.vlen : plan->xbuf;

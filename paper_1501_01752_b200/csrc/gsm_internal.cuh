@@ -61,7 +61,15 @@ struct ApplyGeom {
     double K[3];         // 2 pi / Lambda_a
     int mmin[3];         // lowest order per axis
     double epsb_re, epsb_im;
+    // slot-refill scan (gsm_scan with more points than max_batch): solve b reads x and writes y at an extra offset of
+    // jslot[b] * jstride complex numbers (its own Arnoldi index times the stride between basis vectors); null otherwise
+    const int* jslot;
+    long jstride;
 };
+// extra offset of solve b's x and y (see ApplyGeom.jslot)
+static __device__ __forceinline__ long slot_offset(const ApplyGeom& g, int b) {
+    return g.jslot ? (long)g.jslot[b] * g.jstride : 0L;
+}
 
 struct KrylovDims {
     long vlen;       // 3n complex numbers per vector
@@ -169,6 +177,24 @@ struct KrylovState {   // all device pointers, one entry (or row) per solve of t
     int* nactive;      // [1]
     double* pol;       // [batch][6]
     double* tol;       // [1]
+    // slot-refill scan only
+    int* running;      // [batch] 1 while the slot holds a point whose results have not been recorded yet
+    int* fin;          // [batch] solve finished in this tick: 1 converged, 2 stopped at max_iters
+    int* point;        // [batch] list index of the slot's point
+    int* newv;         // [batch] slot was handed a new point in this tick
+};
+// Device side of a slot-refill scan: the whole point list and the per-point outputs.
+struct RefillDev {
+    const double* kvec_all;   // [npts][3]
+    const double* k0_all;     // [npts]
+    const double* pol_all;    // [npts][6]
+    int npts;
+    int* next;                // [1] first point not handed out yet
+    int* ndone;               // [1] points whose results are recorded
+    int* out_iters;           // [npts]
+    double* out_resid;        // [npts]
+    cplx* out_resp;           // [npts][3]
+    int* out_flag;            // [npts] 1: stopped at max_iters
 };
 cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0 /*index of m=0*/, long n,
                                cudaStream_t st, Profiler* prof);
@@ -177,10 +203,12 @@ cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, 
 cudaError_t launch_sweep_update(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
 cudaError_t launch_givens(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
 cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);
-cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);
+// d_mask (may be null): per-solve flags, solves with mask[b] == 0 are skipped (also in launch_combine / launch_mesh_scatter)
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof,
+                             const int* d_mask = nullptr);
 // E[b] = (guess[b] ? x0[b] : 0) + sum_i y_i v_i; x0 may be null and may alias d_E
 cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_x0, cplx* d_E, cudaStream_t st,
-                           Profiler* prof);
+                           Profiler* prof, const int* d_mask = nullptr);
 // Start from an initial guess (Saad Alg. 6.9 with x0 != 0): given y = A x0 in basis slot 1, set
 // r0 = b - y, beta = ||r0||, v_0 = r0 / beta, g_0 = beta for every solve whose guess beats the zero start
 // (||r0|| < ||b||); the others keep the state launch_krylov_init gave them.
@@ -196,7 +224,12 @@ cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int b
 cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all, const int* d_nbr, const cplx* d_wgt,
                               cplx* d_x0, cudaStream_t st, Profiler* prof);
 cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,
-                                cudaStream_t st, Profiler* prof);
+                                cudaStream_t st, Profiler* prof, const int* d_mask = nullptr);
+// slot-refill scan: mark the solves that finished in this tick; record their results and hand out the next points
+cudaError_t launch_refill_mark(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);
+cudaError_t launch_refill_commit(const KrylovDims& d, const KrylovState& s, const RefillDev& r, int batch, long i0, long n,
+                                 const cplx* d_E_slot, const double* d_resid_slot, double* d_kvec_slot, double* d_k0_slot,
+                                 cudaStream_t st, Profiler* prof);
 // rflag[b] = 0 for the solves whose guess met the stop test without iterating (E = x0 and the true residual is the
 // ||r0|| / ||b|| already formed from A x0), 1 for all others
 cudaError_t launch_residual_select(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof);

@@ -231,9 +231,9 @@ __global__ void __launch_bounds__(KT) normalize_kernel(KrylovDims d, KrylovState
 
 // y = R^{-1} g (upper triangular, m = iters[b]).  One warp per solve: the lanes share each row's sum (row i of R is
 // contiguous in k), fixed shuffle tree, so the m dependent steps cost one load round trip each instead of m - i.
-__global__ void __launch_bounds__(128) backsolve_kernel(KrylovDims d, KrylovState s, int batch) {
+__global__ void __launch_bounds__(128) backsolve_kernel(KrylovDims d, KrylovState s, int batch, const int* __restrict__ mask) {
     const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (b >= batch) return;
+    if (b >= batch || (mask && !mask[b])) return;
     const int m = s.iters[b];
     const cplx* Rc = s.R + (long)b * d.ld * d.mmax;
     const cplx* g = s.g + (long)b * d.ld;
@@ -258,8 +258,10 @@ __global__ void __launch_bounds__(128) backsolve_kernel(KrylovDims d, KrylovStat
 
 // E[b] = x0[b] (if the solve started from a guess) + sum_{i<m} y_i v_i.  x0 may alias out (same thread, same element).
 template <int E>
-__global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s, int batch, const cplx* x0, cplx* out) {
+__global__ void __launch_bounds__(KT) combine_kernel(KrylovDims d, KrylovState s, int batch, const cplx* x0, cplx* out,
+                                                     const int* __restrict__ mask) {
     const int b = blockIdx.y;
+    if (mask && !mask[b]) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* y = reinterpret_cast<cplx*>(smem_raw);
     const int m = s.iters[b];
@@ -399,14 +401,109 @@ __global__ void __launch_bounds__(KT) mesh_guess_kernel(KrylovDims d, const cplx
 }
 template <int E>
 __global__ void __launch_bounds__(KT) mesh_scatter_kernel(KrylovDims d, const cplx* __restrict__ src, const int* __restrict__ idx,
-                                                          cplx* __restrict__ all) {
+                                                          cplx* __restrict__ all, const int* __restrict__ mask) {
     const int b = blockIdx.y;
+    if (mask && !mask[b]) return;
     const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
     cplx* dst = all + (long)idx[b] * d.vlen;
 #pragma unroll
     for (int k = 0; k < E; ++k) {
         const long e = e0 + (long)k * KT;
         if (e < d.vlen) dst[e] = src[(long)b * d.vlen + e];
+    }
+}
+
+// ---- slot-refill scan (gsm_scan with more points than max_batch; the scan is a list of independent
+// solves).  A slot whose solve has finished is given the next pending point at the next tick, so the lock-step batch
+// stays full; every solve is at its own Arnoldi index s.iters[b].
+// After the Arnoldi step of a tick: fin[b] = 1 if the slot's solve converged in this tick, 2 if it stopped at max_iters;
+// rflag[b] (mask of the true-residual apply) = fin[b] != 0.
+__global__ void refill_mark_kernel(KrylovDims d, KrylovState s, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    int f = 0;
+    if (s.running[b]) {
+        if (!s.active[b]) f = 1;
+        else if (s.iters[b] >= d.mmax) { s.active[b] = 0; atomicSub(s.nactive, 1); f = 2; }
+    }
+    s.fin[b] = f;
+    s.rflag[b] = f != 0;
+}
+// One block.  Records the results of the slots that finished (their true residual is in resid_slot, their field in
+// E_slot) under their point index, then hands the next pending points to the free slots in slot order (deterministic)
+// and initialises their Krylov state as krylov_init_kernel does; newv[b] = 1 where v_0 has to be written.
+__global__ void __launch_bounds__(256) refill_commit_kernel(KrylovDims d, KrylovState s, RefillDev r, int batch, long i0, long n,
+                                                            const cplx* __restrict__ E_slot, const double* __restrict__ resid_slot,
+                                                            double* __restrict__ kvec_slot, double* __restrict__ k0_slot) {
+    __shared__ int wcount[8];
+    __shared__ int base_sh;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) base_sh = *r.next;
+    __syncthreads();
+    for (int b0 = 0; b0 < batch; b0 += 256) {
+        const int b = b0 + threadIdx.x;
+        bool want = false;
+        if (b < batch) {
+            if (s.fin[b]) {
+                const int p = s.point[b];
+                r.out_iters[p] = s.iters[b];
+                r.out_resid[p] = resid_slot[b];
+                for (int c = 0; c < 3; ++c) r.out_resp[3 * (long)p + c] = E_slot[(long)b * d.vlen + c * n + i0];
+                r.out_flag[p] = s.fin[b] == 2;
+                s.running[b] = 0;
+                s.fin[b] = 0;
+                atomicAdd(r.ndone, 1);
+            }
+            want = !s.running[b];
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, want);
+        if (lane == 0) wcount[warp] = __popc(m);
+        __syncthreads();
+        int before = __popc(m & ((1u << lane) - 1u)), total = 0;
+        for (int w = 0; w < 8; ++w) { if (w < warp) before += wcount[w]; total += wcount[w]; }
+        const int q = base_sh + before;
+        int nv = 0;
+        if (want && q < r.npts) {
+            s.point[b] = q;
+            for (int a = 0; a < 3; ++a) kvec_slot[3 * b + a] = r.kvec_all[3 * (long)q + a];
+            k0_slot[b] = r.k0_all[q];
+            double* p = s.pol + 6 * b;
+            double bb = 0.0;
+            for (int a = 0; a < 6; ++a) { p[a] = r.pol_all[6 * (long)q + a]; bb += p[a] * p[a]; }
+            const double beta = sqrt(bb);
+            s.beta[b] = beta;
+            s.bnorm[b] = beta;
+            s.guess[b] = 0;
+            s.iters[b] = 0;
+            s.active[b] = beta > 0.0 ? 1 : 0;
+            if (beta > 0.0) atomicAdd(s.nactive, 1);
+            for (int i = 0; i < d.ld; ++i) s.g[(long)b * d.ld + i] = make_double2(0.0, 0.0);
+            s.g[(long)b * d.ld] = make_double2(beta, 0.0);
+            s.running[b] = 1;
+            nv = 1;
+        }
+        if (b < batch) s.newv[b] = nv;
+        __syncthreads();
+        if (threadIdx.x == 0) base_sh = min(base_sh + total, r.npts);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *r.next = base_sh;
+}
+// v_0 = b / ||b|| (the delta vector at m = 0) for the slots that have just been given a point
+template <int E>
+__global__ void __launch_bounds__(KT) refill_v0_kernel(KrylovDims d, KrylovState s, int batch, long i0, long n) {
+    const int b = blockIdx.y;
+    if (!s.newv[b]) return;
+    const double bn = s.bnorm[b];
+    cplx* v0 = s.basis + (long)b * d.vlen;
+    const long e0 = (long)blockIdx.x * (KT * E) + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        const long e = e0 + (long)k * KT;
+        if (e >= d.vlen) continue;
+        const long c = e / n, rr = e - c * n;
+        v0[e] = (rr == i0 && bn > 0.0) ? make_double2(s.pol[6 * b + 2 * c] / bn, s.pol[6 * b + 2 * c + 1] / bn)
+                                       : make_double2(0.0, 0.0);
     }
 }
 
@@ -455,9 +552,10 @@ cudaError_t launch_normalize(const KrylovDims& d, const KrylovState& s, int batc
     normalize_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, j);
     return cudaGetLastError();
 }
-cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
+cudaError_t launch_backsolve(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof,
+                             const int* d_mask) {
     ProfScope ps_(prof, KC_SMALL, st);
-    backsolve_kernel<<<(batch + 3) / 4, 128, 0, st>>>(d, s, batch);
+    backsolve_kernel<<<(batch + 3) / 4, 128, 0, st>>>(d, s, batch, d_mask);
     return cudaGetLastError();
 }
 cudaError_t launch_krylov_guess(const KrylovDims& d, const KrylovState& s, int batch, long i0, long n, cudaStream_t st,
@@ -479,15 +577,29 @@ cudaError_t launch_mesh_guess(const KrylovDims& d, int batch, const cplx* d_all,
     return cudaGetLastError();
 }
 cudaError_t launch_mesh_scatter(const KrylovDims& d, int batch, const cplx* d_src, const int* d_idx, cplx* d_all,
-                                cudaStream_t st, Profiler* prof) {
+                                cudaStream_t st, Profiler* prof, const int* d_mask) {
     ProfScope ps_(prof, KC_SMALL, st);
-    mesh_scatter_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, d_src, d_idx, d_all);
+    mesh_scatter_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, d_src, d_idx, d_all, d_mask);
     return cudaGetLastError();
 }
 cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch, const cplx* d_x0, cplx* d_E, cudaStream_t st,
-                           Profiler* prof) {
+                           Profiler* prof, const int* d_mask) {
     ProfScope ps_(prof, KC_COMBINE, st);   // (m_b + 1) V per solve, billed by run_batch from the iteration counts
-    combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_x0, d_E);
+    combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_x0, d_E, d_mask);
+    return cudaGetLastError();
+}
+cudaError_t launch_refill_mark(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
+    refill_mark_kernel<<<(batch + 127) / 128, 128, 0, st>>>(d, s, batch);
+    return cudaGetLastError();
+}
+cudaError_t launch_refill_commit(const KrylovDims& d, const KrylovState& s, const RefillDev& r, int batch, long i0, long n,
+                                 const cplx* d_E_slot, const double* d_resid_slot, double* d_kvec_slot, double* d_k0_slot,
+                                 cudaStream_t st, Profiler* prof) {
+    { ProfScope ps_(prof, KC_SMALL, st);
+      refill_commit_kernel<<<1, 256, 0, st>>>(d, s, r, batch, i0, n, d_E_slot, d_resid_slot, d_kvec_slot, d_k0_slot); }
+    ProfScope ps2_(prof, KC_NORMALIZE, st);
+    refill_v0_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, 0, st>>>(d, s, batch, i0, n);
     return cudaGetLastError();
 }
 cudaError_t launch_residual_select(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {

@@ -393,3 +393,88 @@ def test_scan_mesh_edge_cases_lossy_hform_short_lists():
         if npts >= 33:            # enough solved points for a pole estimate: the guesses pay (shorter lists: any guess is valid)
             assert it2.sum() < it1.sum()
         plan.close()
+
+
+def test_scan_slot_refill_bit_identical_and_vs_oracle():
+    """gsm_scan from a zero start with more points than max_batch keeps the lock-step batch full: a slot whose solve has
+    finished takes the next pending point, every solve at its own Arnoldi index (the scan is a list
+    of independent solves).  Per solve the arithmetic is that of one lock-step batch: bit-identical results; fields
+    against the oracle's GMRES; E- and H-form; 64-point fast path (17^3) and generic passes (7^3)."""
+    for orders, form in (((17, 17, 17), gsm.FORM_E), ((7, 7, 7), gsm.FORM_E), ((7, 7, 7), gsm.FORM_H)):
+        geo = wl.sphere_lattice(orders)
+        npts = 11
+        kappa = wl.kappa_mesh(1.02, 1.30, npts)
+        kb, kk, pol = wl.scan_points(kappa, 2, 0)
+        kb[3] = [0.3, -0.2, 1.15 * TWO_PI]                       # one off-axis point with a general amplitude
+        pol[3] = [0.2, 0.0, 1.0, 0.0, 0.0, 0.1]
+        pol[7] = 0.0                                              # and one zero source (E = 0, no iterations)
+        one = gsm.plan_from_geometry(geo, max_iters=80, max_batch=16, formulation=form)
+        few = gsm.plan_from_geometry(geo, max_iters=80, max_batch=3, formulation=form)
+        Fa = torch.empty((npts, 3) + orders, dtype=torch.complex128, device="cuda")
+        Fb = torch.zeros_like(Fa)
+        ra, ia, resa, sta = one.scan(kb, kk, pol, tol=1e-12, fields=Fa)
+        rb, ib, resb, stb = few.scan(kb, kk, pol, tol=1e-12, fields=Fb)
+        assert sta == gsm.OK and stb == gsm.OK and len(set(ia.tolist())) > 2
+        assert np.array_equal(ia, ib) and np.array_equal(ra, rb) and np.array_equal(resa, resb)
+        assert torch.equal(Fa, Fb)
+        assert ib[7] == 0 and float(Fb[7].abs().max()) == 0.0 and np.all(resb <= 1e-10)
+        # without a field buffer the responses are the same
+        rc, ic, _, _ = few.scan(kb, kk, pol, tol=1e-12)
+        assert np.array_equal(rc, ra) and np.array_equal(ic, ia)
+        # launch accounting: the refill scan needs fewer Arnoldi launches than three-at-a-time chunks would
+        few.profile_read(reset=True)
+        few.scan(kb, kk, pol, tol=1e-12)
+        launches = few.profile_read()["arnoldi_mgs"][0]
+        chunks = sum(int(ia[p0:p0 + 3].max()) for p0 in range(0, npts, 3))
+        assert launches < chunks + 4
+        if form == gsm.FORM_E:
+            c = coeffs(geo)
+            F = Fb.cpu().numpy()
+            for p in (3, 10):
+                a = pol[p, 0::2] + 1j * pol[p, 1::2]
+                if orders[0] == 7:
+                    ref = orc.solve_dense(c, geo.periods, geo.orders, kb[p], kk[p], geo.eps_b, a)
+                else:
+                    ref, _, _ = orc.solve_gmres(c, geo.periods, geo.orders, kb[p], kk[p], geo.eps_b, a, tol=1e-13,
+                                                max_iters=120, matvec=orc.toeplitz_matvec_c)
+                assert rel(F[p], ref) <= 1e-9
+        one.close(); few.close()
+
+
+def test_scan_slot_refill_max_iters_and_single_slot():
+    """Refill with one slot (max_batch 1) and a basis too small to converge: every point stops at max_iters with the best
+    iterate and the scan reports GSM_NOT_CONVERGED; with room to converge the single slot reproduces gsm_solve."""
+    geo = wl.sphere_lattice((7, 7, 7))
+    kappa = wl.kappa_mesh(1.05, 1.25, 5)
+    kb, kk, pol = wl.scan_points(kappa, 2, 0)
+    short = gsm.plan_from_geometry(geo, max_iters=4, max_batch=2)
+    _, it, res, st = short.scan(kb, kk, pol, tol=1e-12)
+    assert st == gsm.NOT_CONVERGED and np.all(it == 4) and np.all(res > 1e-12) and np.all(res < 1.0)
+    short.close()
+    plan = gsm.plan_from_geometry(geo, max_iters=64, max_batch=1)
+    F = torch.empty((5, 3, 7, 7, 7), dtype=torch.complex128, device="cuda")
+    _, it, res, st = plan.scan(kb, kk, pol, tol=1e-12, fields=F)
+    assert st == gsm.OK
+    for p in range(5):
+        E, _, iters, resid, _ = plan.solve(kb[p], kk[p], pol[p, 0::2] + 1j * pol[p, 1::2], tol=1e-12)
+        assert iters == it[p] and resid == res[p] and torch.equal(E, F[p])
+    plan.close()
+
+
+def test_cluster_gram_schmidt_at_32_cubed():
+    """32^3 orders (98 304 complex numbers per vector = 6144 per CTA of a 16-CTA cluster) is the largest vector the cluster
+    Gram-Schmidt kernel holds on chip; it agrees with the two-sweep kernels and the field satisfies the equation at
+    sampled harmonics (the oracle's O(n) row sums)."""
+    from test_gpu_solve import _check_equation_rows
+    geo = wl.sphere_lattice((32, 32, 32))
+    kb, pol = np.array([0.0, 0.0, 1.2 * TWO_PI]), np.array([1.0, 0.0, 0.0], dtype=complex)
+    plan = gsm.plan_from_geometry(geo, max_iters=80)
+    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    prof = plan.profile_read()
+    assert st == gsm.OK and resid <= 1e-10 and prof["arnoldi_mgs"][0] >= iters and prof["sweep_dots"][0] == 0
+    plan.close()
+    two = gsm.plan_from_geometry(geo, max_iters=80, flags=gsm.FLAG_TWO_SWEEP)
+    E2, _, it2, res2, st2 = two.solve(kb, TWO_PI, pol, tol=1e-12)
+    assert st2 == gsm.OK and abs(it2 - iters) <= 1 and rel(E.cpu().numpy(), E2.cpu().numpy()) <= 1e-10
+    two.close()
+    _check_equation_rows(geo, coeffs(geo), E.cpu().numpy()[None], kb[None], np.array([TWO_PI]), pol[None], 6)

@@ -316,7 +316,7 @@ def _check_equation_rows(geo, c, F, kb, k0, pol, nsamp):
     """(A E)_m = b_m at sampled harmonics, A E evaluated by the oracle's row sum (no FFT, O(n) per row)."""
     rng = np.random.default_rng(17)
     N = geo.orders
-    i0 = tuple((n - 1) // 2 for n in N)
+    i0 = tuple(n // 2 for n in N)             # index of m = 0 (reading R1: odd N: (N-1)/2, even N: N/2)
     for b in range(F.shape[0]):
         k = orc.wavevectors(geo.periods, N, kb[b])
         kb2 = k0[b] ** 2 * geo.eps_b
