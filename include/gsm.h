@@ -56,13 +56,17 @@ enum { GSM_SPHERE = 0, GSM_ELLIPSOID = 1, GSM_BOX = 2, GSM_POLYHEDRON = 3 };
  *       voxel path: transform of 1 - eps_b/eps_j.  gsm_plan_coeffs returns D_d.  `pol` is the amplitude h of H^inc. */
 enum { GSM_FORM_E = 0, GSM_FORM_H = 1 };
 
-/* Diagnostic flags of a plan (gsm_plan_desc.flags, 0 in normal use).  They select the general-purpose code path where
- * a specialised one would be taken, so that tests can hold both to the same parity bar:
+/* Flags of a plan (gsm_plan_desc.flags, 0 in normal use).  They select an alternative code path where a default one
+ * exists, so that tests can hold both to the same parity bar:
  *   GSM_FLAG_TWO_SWEEP     Gram-Schmidt by the two-sweep kernels even where one field vector fits a thread-block cluster
  *   GSM_FLAG_GENERIC_APPLY generic radix-2/4/8 FFT passes even where a 64- or 128-point fast path applies
  *   GSM_FLAG_FUSED_APPLY   64-point fast path as ONE persistent launch that keeps the z-transformed intermediate in L2
- *                          (apply_fused64.cu) instead of three launches through HBM; measured slower */
-enum { GSM_FLAG_TWO_SWEEP = 1, GSM_FLAG_GENERIC_APPLY = 2, GSM_FLAG_FUSED_APPLY = 4 };
+ *                          (apply_fused64.cu) instead of three launches through HBM; measured slower
+ *   GSM_FLAG_SLOT_REFILL   gsm_scan from a zero start with more points than max_batch: instead of solving max_batch points,
+ *                          draining, and taking the next max_batch, a slot whose solve has finished is handed the next pending
+ *                          point at once (every solve at its own Arnoldi index).  Same results bit for bit; measured neutral
+ *                          to slightly slower on the 31^3 workload, where the draining ticks are cheap */
+enum { GSM_FLAG_TWO_SWEEP = 1, GSM_FLAG_GENERIC_APPLY = 2, GSM_FLAG_FUSED_APPLY = 4, GSM_FLAG_SLOT_REFILL = 8 };
 
 #define GSM_MAX_ITERS 512   /* largest accepted gsm_plan_desc.max_iters */
 

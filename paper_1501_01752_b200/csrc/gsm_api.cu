@@ -350,7 +350,7 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         return fail(nullptr, GSM_E_INVALID, "shapes missing");
     // the two-sweep kernels stage (j + 1)-sized rows in shared memory and the pool holds max_iters + 1 vectors per solve
     if (desc->max_iters > GSM_MAX_ITERS) return fail(nullptr, GSM_E_INVALID, "max_iters exceeds GSM_MAX_ITERS");
-    if (desc->flags & ~(GSM_FLAG_TWO_SWEEP | GSM_FLAG_GENERIC_APPLY | GSM_FLAG_FUSED_APPLY))
+    if (desc->flags & ~(GSM_FLAG_TWO_SWEEP | GSM_FLAG_GENERIC_APPLY | GSM_FLAG_FUSED_APPLY | GSM_FLAG_SLOT_REFILL))
         return fail(nullptr, GSM_E_INVALID, "unknown flag");
     gsm_plan* plan = new (std::nothrow) gsm_plan();
     if (!plan) return fail(nullptr, GSM_E_ALLOC, "host allocation failed");
@@ -760,7 +760,7 @@ extern "C" gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_b
     if (!plan) return GSM_E_INVALID;
     if (npts < 0 || !k_bloch || !k0 || !pol || !(tol > 0.0)) return fail(plan, GSM_E_INVALID, "gsm_scan: bad argument");
     bool nc = false;
-    if (!d_x0 && npts > plan->max_batch && plan->mgs_cs > 0 && !plan->fused.ring) {   // keep the lock-step batch full
+    if ((plan->desc.flags & GSM_FLAG_SLOT_REFILL) && !d_x0 && npts > plan->max_batch && plan->mgs_cs > 0 && !plan->fused.ring) {
         gsm_status s = run_refill(plan, npts, k_bloch, k0, pol, tol, static_cast<cplx*>(d_E_out), resp_host, iters, resid, &nc);
         if (s != GSM_OK) return s;
         return nc ? GSM_NOT_CONVERGED : GSM_OK;

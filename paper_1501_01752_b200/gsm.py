@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libgsm_b200.so")
 OK, NOT_CONVERGED, E_INVALID, E_ALLOC, E_CUDA, E_SINGULAR_BASIS = 0, 1, -1, -2, -3, -4
 SPHERE, ELLIPSOID, BOX, POLYHEDRON = 0, 1, 2, 3
 FORM_E, FORM_H = 0, 1
-FLAG_TWO_SWEEP, FLAG_GENERIC_APPLY, FLAG_FUSED_APPLY = 1, 2, 4   # diagnostics (include/gsm.h GSM_FLAG_*)
+FLAG_TWO_SWEEP, FLAG_GENERIC_APPLY, FLAG_FUSED_APPLY, FLAG_SLOT_REFILL = 1, 2, 4, 8   # include/gsm.h GSM_FLAG_*
 MAX_ITERS = 512
 
 

@@ -396,7 +396,7 @@ def test_scan_mesh_edge_cases_lossy_hform_short_lists():
 
 
 def test_scan_slot_refill_bit_identical_and_vs_oracle():
-    """gsm_scan from a zero start with more points than max_batch keeps the lock-step batch full: a slot whose solve has
+    """GSM_FLAG_SLOT_REFILL: gsm_scan from a zero start with more points than max_batch keeps the lock-step batch full: a slot whose solve has
     finished takes the next pending point, every solve at its own Arnoldi index (the scan is a list
     of independent solves).  Per solve the arithmetic is that of one lock-step batch: bit-identical results; fields
     against the oracle's GMRES; E- and H-form; 64-point fast path (17^3) and generic passes (7^3)."""
@@ -409,7 +409,7 @@ def test_scan_slot_refill_bit_identical_and_vs_oracle():
         pol[3] = [0.2, 0.0, 1.0, 0.0, 0.0, 0.1]
         pol[7] = 0.0                                              # and one zero source (E = 0, no iterations)
         one = gsm.plan_from_geometry(geo, max_iters=80, max_batch=16, formulation=form)
-        few = gsm.plan_from_geometry(geo, max_iters=80, max_batch=3, formulation=form)
+        few = gsm.plan_from_geometry(geo, max_iters=80, max_batch=3, formulation=form, flags=gsm.FLAG_SLOT_REFILL)
         Fa = torch.empty((npts, 3) + orders, dtype=torch.complex128, device="cuda")
         Fb = torch.zeros_like(Fa)
         ra, ia, resa, sta = one.scan(kb, kk, pol, tol=1e-12, fields=Fa)
@@ -447,11 +447,11 @@ def test_scan_slot_refill_max_iters_and_single_slot():
     geo = wl.sphere_lattice((7, 7, 7))
     kappa = wl.kappa_mesh(1.05, 1.25, 5)
     kb, kk, pol = wl.scan_points(kappa, 2, 0)
-    short = gsm.plan_from_geometry(geo, max_iters=4, max_batch=2)
+    short = gsm.plan_from_geometry(geo, max_iters=4, max_batch=2, flags=gsm.FLAG_SLOT_REFILL)
     _, it, res, st = short.scan(kb, kk, pol, tol=1e-12)
     assert st == gsm.NOT_CONVERGED and np.all(it == 4) and np.all(res > 1e-12) and np.all(res < 1.0)
     short.close()
-    plan = gsm.plan_from_geometry(geo, max_iters=64, max_batch=1)
+    plan = gsm.plan_from_geometry(geo, max_iters=64, max_batch=1, flags=gsm.FLAG_SLOT_REFILL)
     F = torch.empty((5, 3, 7, 7, 7), dtype=torch.complex128, device="cuda")
     _, it, res, st = plan.scan(kb, kk, pol, tol=1e-12, fields=F)
     assert st == gsm.OK
