@@ -162,6 +162,29 @@ def oracle_apply_once(geo, kb, k0, reps=3):
     return (time.perf_counter() - t0) / reps
 
 
+def oracle_small_sizes():
+    """the oracle as it stands at the smaller configs - one operator apply and one full GMRES solve each
+    (7^3 sphere, 1x1x63 laminate, 15^3 ellipsoid); seconds.  63^3 is not run: 1.9e11 complex MACs per apply."""
+    from oracle import gsm_oracle as orc
+    from paper_1501_01752_b200 import workloads as wl
+    out = []
+    for name, geo, kbv, k0v in (("7^3 sphere (cfg 1)", wl.sphere_lattice((7, 7, 7)), [0.0, 0.0, 1.2 * TWO_PI], TWO_PI),
+                                ("1x1x63 laminate (cfg 2)", wl.laminate(), [0.0, 0.0, 0.9], 0.5),
+                                ("15^3 ellipsoid (cfg 3)", wl.ellipsoid_lattice(), [0.0, 0.0, 1.1 * TWO_PI], TWO_PI)):
+        c = orc.coeffs_analytic(geo.periods, geo.orders, geo.shapes, geo.eps_bg, geo.eps_b)
+        kbv = np.asarray(kbv)
+        x = wl.random_field(1, geo.orders)[0]
+        orc.apply_operator(c, x, geo.periods, kbv, k0v, geo.eps_b, orc.toeplitz_matvec_c)
+        t0 = time.perf_counter()
+        orc.apply_operator(c, x, geo.periods, kbv, k0v, geo.eps_b, orc.toeplitz_matvec_c)
+        t_apply = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        _, _, its = orc.solve_gmres(c, geo.periods, geo.orders, kbv, k0v, geo.eps_b, np.array([1.0, 0, 0], dtype=complex),
+                                    tol=TOL, max_iters=200, matvec=orc.toeplitz_matvec_c)
+        out.append({"workload": name, "apply_s": t_apply, "solve_s": time.perf_counter() - t0, "iters": int(its)})
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -366,6 +389,17 @@ def run_gsm(args):
         a1.record(stream)
     barrier()
     apply_ms = max_over_ranks(a0.elapsed_time(a1)) / napply
+    # one solve's apply alone (SURVEY 8(d) "single and batch-256"): x, y, W and Chat (~13 MB) stay in L2
+    with torch.cuda.stream(stream):
+        for _ in range(3):
+            plan.apply(kb[:1], k0[:1], x[:1], out=y[:1])
+        barrier()
+        a0.record(stream)
+        for _ in range(200):
+            plan.apply(kb[:1], k0[:1], x[:1], out=y[:1])
+        a1.record(stream)
+    barrier()
+    apply1_ms = a0.elapsed_time(a1) / 200
     V = 16.0 * 3 * geo.n
     chat_bytes = 16.0 * 64 ** 3
     apply_alg_bytes = 2 * V * BATCH + chat_bytes
@@ -466,6 +500,7 @@ def run_gsm(args):
     # ---- CPU oracle on a bounded sample ---------------------------------------------------------------------------
     cpu_t, cpu_it, cores = oracle_solve_once(geo, kb[0], k0[0], pol[0])
     cpu_apply_t = oracle_apply_once(geo, kb[0], k0[0])
+    cpu_small = oracle_small_sizes()
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -492,7 +527,10 @@ def run_gsm(args):
         "kernel_GBps": k_gbs,
         "applies_per_s": BATCH * world / (apply_ms * 1e-3),
         "apply": {"ms_per_batch_apply": apply_ms, "algorithmic_GBps": apply_alg_bytes / (apply_ms * 1e-3) / 1e9,
-                  "frac": apply_alg_bytes / (apply_ms * 1e-3) / 1e9 / peak, "definition": "(2V x 256 + |Chat|) / time"},
+                  "frac": apply_alg_bytes / (apply_ms * 1e-3) / 1e9 / peak, "definition": "(2V x 256 + |Chat|) / time",
+                  "single_apply_us": 1e3 * apply1_ms,
+                  "single_apply_note": "batch of 1: three launches whose working set (x, y, W, Chat ~ 13 MB) stays in L2; "
+                                       "latency-bound, no HBM figure is meaningful (SURVEY 8(d))"},
         "lockstep_zero_start": {"value": BATCH * world / (z_ms * 1e-3), "unit": UNIT, "ms_per_step": z_ms,
                                 "mean_iters": float(np.mean(z_iters)), "max_true_resid": float(np.max(z_resid)),
                                 "note": "plain gsm_scan: all 256 points in one lock-step batch from x0 = 0; every launch "
@@ -514,7 +552,8 @@ def run_gsm(args):
                                    f"{cpu_it} iterations, {cpu_t:.1f} s)",
                          "applies_per_s": 1.0 / cpu_apply_t,
                          "apply_sample": f"one operator apply at 31^3 orders (O(n^2) Toeplitz product + Green dyadic), "
-                                         f"mean of 3, {cpu_apply_t:.2f} s"},
+                                         f"mean of 3, {cpu_apply_t:.2f} s",
+                         "other_sizes": cpu_small},
     }
     print(json.dumps(line), flush=True)
     if world > 1:

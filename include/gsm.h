@@ -152,6 +152,12 @@ gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch, const dou
 gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double k0, const double pol[6], double tol,
                      void* d_E_out, double* resid_hist_host, int hist_cap, int* n_iters, double* true_rel_resid);
 
+/* Residual history of one solve of the most recent lock-step batch (gsm_solve: b = 0; gsm_scan / gsm_scan_guess with
+ * npts <= max_batch: b = list index; longer lists and gsm_scan_mesh run several batches, of which the last is kept):
+ * the first min(n_iters, hist_cap) residual estimates |g_{j+1}| / ||b|| and *n_iters.
+ * GSM_E_INVALID if b is not a solve of that batch. */
+gsm_status gsm_plan_history(gsm_plan* plan, int b, double* resid_hist_host, int hist_cap, int* n_iters);
+
 /* Scan: npts independent solves sharing the plan, run max_batch at a time in lock step.
  * resp_host[npts][3] complex = E at m = 0; iters[npts]; resid[npts] = true relative residuals.
  * d_E_out (may be NULL): device, [npts][3][N1][N2][N3] complex, all fields. */

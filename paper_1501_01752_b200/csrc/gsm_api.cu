@@ -19,6 +19,7 @@ struct gsm_plan {
     KrylovState ks{};
     cudaStream_t stream = nullptr;
     int max_batch = 1, max_iters = 64;
+    int last_nb = 0;              // size of the most recent lock-step batch (gsm_plan_history)
     long i0 = 0;                  // flat index of m = 0 inside one component
     int mgs_cs = 0, mgs_chunk = 0, mgs_nclusters = 0; // cluster MGS Arnoldi step (0 = two-sweep fallback)
     Fused64Dev fused;             // fused persistent apply for 64-point axes (ring == null: three-launch apply)
@@ -565,6 +566,7 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     const ApplyGeom& g = plan->geom;
     cudaStream_t st = plan->stream;
     if (singular_basis(plan, nb, kvec, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
+    plan->last_nb = nb;
     double* pin = static_cast<double*>(plan->pinned);
     int* pin_i = reinterpret_cast<int*>(pin);           // [0] nactive; then staging
     CK(cudaMemcpyAsync(plan->d_kvec, kvec, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, st));
@@ -666,6 +668,7 @@ static gsm_status run_refill(gsm_plan* plan, int npts, const double* kvec, const
     Profiler* prof = &plan->prof;
     const int B = plan->max_batch;
     if (singular_basis(plan, npts, kvec, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
+    plan->last_nb = 0;   // slots are reused: no per-solve history is kept
     // device copy of the list and per-point outputs: [resp 6][kvec 3][k0 1][pol 6][resid 1] doubles, [iters][flag] ints
     const size_t per_pt = sizeof(double) * 17 + sizeof(int) * 2;
     if (plan->refill_cap < (size_t)npts) {
@@ -752,6 +755,20 @@ extern "C" gsm_status gsm_solve(gsm_plan* plan, const double k_bloch[3], double 
                              true_rel_resid, resid_hist_host, hist_cap, &nc);
     if (s != GSM_OK) return s;
     return nc ? GSM_NOT_CONVERGED : GSM_OK;
+}
+
+extern "C" gsm_status gsm_plan_history(gsm_plan* plan, int b, double* resid_hist_host, int hist_cap, int* n_iters) {
+    if (!plan) return GSM_E_INVALID;
+    if (b < 0 || b >= plan->last_nb || hist_cap < 0 || (hist_cap > 0 && !resid_hist_host) || !n_iters)
+        return fail(plan, GSM_E_INVALID, "gsm_plan_history: bad argument or no such solve in the last batch");
+    CK(cudaStreamSynchronize(plan->stream));
+    int m = 0;
+    CK(cudaMemcpy(&m, plan->ks.iters + b, sizeof(int), cudaMemcpyDeviceToHost));
+    const int cnt = std::min(std::min(hist_cap, plan->kd.mmax), m);
+    if (cnt > 0)
+        CK(cudaMemcpy(resid_hist_host, plan->ks.hist + (size_t)b * plan->kd.mmax, sizeof(double) * cnt, cudaMemcpyDeviceToHost));
+    *n_iters = m;
+    return GSM_OK;
 }
 
 extern "C" gsm_status gsm_scan_guess(gsm_plan* plan, int npts, const double* k_bloch, const double* k0, const double* pol,

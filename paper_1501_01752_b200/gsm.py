@@ -59,6 +59,8 @@ def _load():
     lib.gsm_plan_info.argtypes = [P, ip, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.gsm_apply.argtypes = [P, C.c_int, P, P, P, P]
     lib.gsm_solve.argtypes = [P, P, C.c_double, P, C.c_double, P, P, C.c_int, ip, dp]
+    lib.gsm_plan_history.argtypes = [P, C.c_int, P, C.c_int, ip]
+    lib.gsm_plan_history.restype = C.c_int
     lib.gsm_scan.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P]
     lib.gsm_scan_guess.argtypes = [P, C.c_int, P, P, P, C.c_double, P, P, P, P, P]
     lib.gsm_scan_mesh.argtypes = [P, C.c_int, P, P, P, C.c_double, C.c_int, P, P, P, P]
@@ -247,6 +249,13 @@ class Plan:
         st = _check(_lib.gsm_solve(self._h, kb.ctypes.data, float(k0), pl.ctypes.data, float(tol), E.data_ptr(),
                                    hist.ctypes.data, self.max_iters, C.byref(it), C.byref(res)), self._h)
         return E, hist[: it.value].copy(), it.value, res.value, st
+
+    def history(self, b=0):
+        """gsm_plan_history: residual estimates of solve b of the most recent lock-step batch."""
+        hist = np.zeros(self.max_iters)
+        it = C.c_int()
+        _check(_lib.gsm_plan_history(self._h, int(b), hist.ctypes.data, self.max_iters, C.byref(it)), self._h)
+        return hist[: it.value].copy()
 
     def scan(self, k_bloch, k0, pol, tol=1e-10, fields=None, x0=None, levels=None):
         """gsm_scan: returns (resp [npts,3] complex, iters [npts], resid [npts], status).

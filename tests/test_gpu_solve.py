@@ -171,6 +171,13 @@ def test_scan_mixed_convergence_and_repeatability():
     rb, ib, _, _ = pb.scan(kb, kk, pol, tol=1e-11)
     assert len(set(ia.tolist())) > 1
     assert np.array_equal(ia, ib) and np.array_equal(ra, rb)      # deterministic reductions: bit-identical
+    # residual history of every solve of the batch (gsm_plan_history), against gsm_solve's own history of that point
+    for b in (0, 5, 11):
+        h = pa.history(b)
+        _, hs, its, _, _ = pb.solve(kb[b], kk[b], pol[b, 0::2] + 1j * pol[b, 1::2], tol=1e-11)
+        assert len(h) == ia[b] == its and np.array_equal(h, hs) and h[-1] <= 1e-11 < h[-2]
+    with pytest.raises(gsm.GsmError):
+        pa.history(12)
     pa.close(); pb.close()
 
 

@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol(lib_path):
     names = declared_functions()
     assert {"gsm_plan_create", "gsm_plan_destroy", "gsm_apply", "gsm_solve", "gsm_scan", "gsm_pole_search",
             "gsm_plan_set_cell", "gsm_plan_profile", "gsm_plan_profile_read", "gsm_last_error", "gsm_scan_guess",
-            "gsm_scan_mesh", "gsm_retrieve_neff_many", "gsm_mesh_schedule"} <= set(names)
+            "gsm_scan_mesh", "gsm_retrieve_neff_many", "gsm_mesh_schedule", "gsm_plan_history"} <= set(names)
     lib = ctypes.CDLL(lib_path)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/gsm.h but not exported by {lib_path}"
