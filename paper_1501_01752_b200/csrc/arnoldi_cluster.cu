@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(MGS_T, 1) arnoldi_mgs_kernel(KrylovDims d, Kry
     const long lo = (long)rank * chunk;
     const int len = (int)max(0L, min((long)chunk, d.vlen - lo));
     const uint32_t bytes = (uint32_t)len * (uint32_t)sizeof(cplx);
-    const long vs = (long)batch * d.vlen;
+    const long vs = d.vstride ? d.vstride : (long)batch * d.vlen;
 
     if (t == 0) {
         mbar_init(&sm->mbar[0], 1);
@@ -283,6 +283,9 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     if (e != cudaSuccess || nclusters < 1) { cudaGetLastError(); return cudaSuccess; }
     *cs_out = cs;
     *chunk_out = chunk;
+#ifdef MGS_NCL_CAP   // tuning experiments only
+    if (nclusters > MGS_NCL_CAP) nclusters = MGS_NCL_CAP;
+#endif
     *nclusters_out = nclusters;
     return cudaSuccess;
 }

@@ -27,6 +27,12 @@ struct gsm_plan {
     long long device_bytes = 0;
     Profiler prof;
     cudaEvent_t iter_ev[2] = {nullptr, nullptr};   // completion of the per-iteration nactive read-back
+    // groups of one lock-step batch iterating concurrently (run_batch): group 0 on `stream`, the others on streams of their own
+    cudaStream_t gstream[GSM_MAX_GROUPS] = {};
+    cudaEvent_t gev[GSM_MAX_GROUPS][2] = {};       // per-group read-back events
+    cudaEvent_t gsync[GSM_MAX_GROUPS] = {};        // fork ([0]) / join
+    int* d_gcount = nullptr;                       // [GSM_MAX_GROUPS] solves of each group still iterating
+
     cplx* chat64 = nullptr;
     cplx* chat128 = nullptr;
     int* gen128[2] = {nullptr, nullptr};
@@ -461,10 +467,17 @@ extern "C" gsm_status gsm_plan_create(const gsm_plan_desc* desc, gsm_plan** out)
         CK(dalloc(plan, &plan->d_kvec, (size_t)B * 3));
         CK(dalloc(plan, &plan->d_k0, (size_t)B));
         CK(dalloc(plan, &plan->d_resid, (size_t)B));
-        plan->pinned_bytes = sizeof(double) * ((size_t)B * (12 + kd.mmax) + 16);
+        plan->pinned_bytes = sizeof(double) * ((size_t)B * (12 + kd.mmax) + 16);   // + 16: per-group read-back slots
         CK(cudaMallocHost(&plan->pinned, plan->pinned_bytes));
         CK(cudaEventCreateWithFlags(&plan->iter_ev[0], cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&plan->iter_ev[1], cudaEventDisableTiming));
+        CK(dalloc(plan, &plan->d_gcount, (size_t)GSM_MAX_GROUPS));
+        for (int q = 0; q < GSM_MAX_GROUPS; ++q) {
+            if (q > 0) CK(cudaStreamCreateWithFlags(&plan->gstream[q], cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&plan->gev[q][0], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&plan->gev[q][1], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&plan->gsync[q], cudaEventDisableTiming));
+        }
         return GSM_OK;
     };
     st = body();
@@ -482,6 +495,11 @@ extern "C" gsm_status gsm_plan_destroy(gsm_plan* plan) {
     cudaStreamSynchronize(plan->stream);
     plan->prof.destroy();
     for (cudaEvent_t e : plan->iter_ev) if (e) cudaEventDestroy(e);
+    for (int q = 0; q < GSM_MAX_GROUPS; ++q) {
+        if (plan->gstream[q]) { cudaStreamSynchronize(plan->gstream[q]); cudaStreamDestroy(plan->gstream[q]); }
+        for (cudaEvent_t e : plan->gev[q]) if (e) cudaEventDestroy(e);
+        if (plan->gsync[q]) cudaEventDestroy(plan->gsync[q]);
+    }
     for (void* p : plan->allocs) cudaFree(p);
     if (plan->mesh_fields) cudaFree(plan->mesh_fields);
     if (plan->refill_buf) cudaFree(plan->refill_buf);
@@ -568,7 +586,6 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     if (singular_basis(plan, nb, kvec, k0)) return fail(plan, GSM_E_SINGULAR_BASIS, "k_m.k_m == k_b^2 for some m");
     plan->last_nb = nb;
     double* pin = static_cast<double*>(plan->pinned);
-    int* pin_i = reinterpret_cast<int*>(pin);           // [0] nactive; then staging
     CK(cudaMemcpyAsync(plan->d_kvec, kvec, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(plan->d_k0, k0, sizeof(double) * nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ks.pol, pol, sizeof(double) * 6 * nb, cudaMemcpyHostToDevice, st));
@@ -585,28 +602,67 @@ static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const do
     }
     // Launches of the iteration loop are billed (algorithmic bytes) after the batch, from the final iteration counts:
     // the host learns how many solves were still iterating one iteration late.
-    int j = 0;
-    for (; j < kd.mmax; ++j) {
-        CK(launch_apply(g, nb, plan->d_kvec, plan->d_k0, ks.basis + (size_t)j * vs, ks.basis + (size_t)(j + 1) * vs,
-                        plan->W, &plan->fused, ks.active, st, prof, 0.0));
-        if (plan->mgs_cs > 0) {
-            CK(launch_arnoldi_cluster(kd, ks, nb, j, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, st, prof));
-        } else {
-            CK(launch_sweep_dots(kd, ks, nb, j, st, prof));
-            CK(launch_hsolve(kd, ks, nb, j, st, prof));
-            CK(launch_sweep_update(kd, ks, nb, j, st, prof));
-            CK(launch_givens(kd, ks, nb, j, st, prof));
-            CK(launch_normalize(kd, ks, nb, j, st, prof));
+    //
+    // Groups.  The Arnoldi kernel is HBM-bound and its clusters occupy 112 of the 148 SMs; the plane convolution of the
+    // apply is bound by the fp64 and shared-memory pipes and leaves HBM idle; and small batches leave every kernel
+    // latency-bound.  The batch is therefore cut into up to GSM_MAX_GROUPS groups of consecutive solves that iterate on
+    // streams of their own, so that one group's Gram-Schmidt runs beside another group's apply (the groups drift apart
+    // by themselves; forcing a stagger, or a high-priority stream for the Gram-Schmidt launches, changes nothing).
+    // Per solve nothing changes (same kernels, same reductions: bit-identical results).  One group when per-launch
+    // profiling is on (clean kernel times), on the two-sweep and fused-apply paths, and below 8 solves.
+    int G = 1;   // measured at 31^3 (ms per scan, 1 / 2 / 4 groups): 16 solves 11.1 / 9.7 / 9.1, 64: 35.4 / 32.2 / 32.9, 256: 129 / 125 / 127
+    if (plan->mgs_cs > 0 && !plan->fused.ring && !prof->on && nb >= 8) G = nb >= 48 ? 2 : std::min(GSM_MAX_GROUPS, nb / 4);
+    GroupBounds gb{};
+    for (int q = 0; q <= G; ++q) gb.b[q] = (int)((long)nb * q / G);
+    KrylovDims kdg = kd;
+    kdg.vstride = (long)vs;
+    int* gpin = reinterpret_cast<int*>(pin + (size_t)plan->max_batch * (12 + kd.mmax));   // [group][parity]
+    if (G > 1) {
+        CK(launch_group_count(ks, G, gb, plan->d_gcount, st, prof));
+        CK(cudaEventRecord(plan->gsync[0], st));
+        for (int q = 1; q < G; ++q) CK(cudaStreamWaitEvent(plan->gstream[q], plan->gsync[0], 0));
+    }
+    bool done[GSM_MAX_GROUPS] = {};
+    for (int j = 0; j < kd.mmax; ++j) {
+        for (int q = 0; q < G; ++q) {
+            if (done[q]) continue;
+            const int b0 = gb.b[q], gn = gb.b[q + 1] - b0;
+            cudaStream_t sq = q == 0 ? st : plan->gstream[q];
+            const KrylovState kq = G > 1 ? krylov_state_view(kd, ks, b0, plan->d_gcount + q) : ks;
+            ApplyGeom gq = g;
+            if (gq.Y) gq.Y += (size_t)b0 * 3 * g.ax[2].P * g.N1 * g.ax[1].P;
+            cplx* Wq = plan->W ? plan->W + (size_t)b0 * 3 * g.ax[2].P * g.NL : nullptr;
+            const cplx* xq = ks.basis + (size_t)j * vs + (size_t)b0 * kd.vlen;
+            CK(launch_apply(gq, gn, plan->d_kvec + 3 * b0, plan->d_k0 + b0, xq, const_cast<cplx*>(xq) + vs, Wq, &plan->fused,
+                            kq.active, sq, prof, 0.0));
+            if (plan->mgs_cs > 0) {
+                CK(launch_arnoldi_cluster(kdg, kq, gn, j, plan->mgs_cs, plan->mgs_chunk, plan->mgs_nclusters, sq, prof));
+            } else {
+                CK(launch_sweep_dots(kd, ks, nb, j, st, prof));
+                CK(launch_hsolve(kd, ks, nb, j, st, prof));
+                CK(launch_sweep_update(kd, ks, nb, j, st, prof));
+                CK(launch_givens(kd, ks, nb, j, st, prof));
+                CK(launch_normalize(kd, ks, nb, j, st, prof));
+            }
+            // The count of solves still iterating comes back one iteration late: iteration j + 1 is enqueued before the
+            // host looks at the count after iteration j - 1, so launches never wait for a round trip.  If everything had
+            // already converged, the extra iteration's CTAs find their `active` flags cleared and exit at once.
+            CK(cudaMemcpyAsync(gpin + 2 * q + (j & 1), kq.nactive, sizeof(int), cudaMemcpyDeviceToHost, sq));
+            CK(cudaEventRecord(plan->gev[q][j & 1], sq));
         }
-        // The count of solves still iterating comes back one iteration late: iteration j + 1 is enqueued before the
-        // host looks at the count after iteration j - 1, so launches never wait for a round trip.  If everything had
-        // already converged, the extra iteration's CTAs find their `active` flags cleared and exit at once.
-        CK(cudaMemcpyAsync(pin_i + (j & 1), ks.nactive, sizeof(int), cudaMemcpyDeviceToHost, st));
-        CK(cudaEventRecord(plan->iter_ev[j & 1], st));
-        if (j >= 1) {
-            CK(cudaEventSynchronize(plan->iter_ev[(j - 1) & 1]));
-            if (pin_i[(j - 1) & 1] <= 0) break;
+        bool all = true;
+        for (int q = 0; q < G; ++q) {
+            if (!done[q] && j >= 1) {
+                CK(cudaEventSynchronize(plan->gev[q][(j - 1) & 1]));
+                if (gpin[2 * q + ((j - 1) & 1)] <= 0) done[q] = true;
+            }
+            all = all && done[q];
         }
+        if (all) break;
+    }
+    for (int q = 1; q < G; ++q) {   // join
+        CK(cudaEventRecord(plan->gsync[q], plan->gstream[q]));
+        CK(cudaStreamWaitEvent(st, plan->gsync[q], 0));
     }
     CK(launch_backsolve(kd, ks, nb, st, prof));
     CK(launch_combine(kd, ks, nb, d_x0, d_E, st, prof));

@@ -77,7 +77,10 @@ struct KrylovDims {
     int chunk;       // elements per CTA (= threads * elems per thread)
     int mmax;        // max iterations (basis holds mmax+1 vectors)
     int ld;          // mmax + 1
+    long vstride;    // complex numbers between consecutive basis vectors of one solve; 0 = batch * vlen (the kernels'
+                     // `batch` argument); set when a launch covers only a group of the batch's solves
 };
+#define GSM_MAX_GROUPS 4   // sub-batches of one lock-step batch that iterate on streams of their own (gsm_api.cu run_batch)
 
 // Device state of the fused persistent apply for 64-point axes (apply_fused64.cu); ring == null: not in use.
 struct Fused64Dev {
@@ -196,6 +199,11 @@ struct RefillDev {
     cplx* out_resp;           // [npts][3]
     int* out_flag;            // [npts] 1: stopped at max_iters
 };
+// view of the per-solve state that starts at solve b0 (every array advanced by b0 entries / rows); nactive = counter
+KrylovState krylov_state_view(const KrylovDims& d, const KrylovState& s, int b0, int* nactive);
+// counts[g] = number of active solves in [bounds[g], bounds[g + 1]), g < ngroups <= GSM_MAX_GROUPS
+struct GroupBounds { int b[GSM_MAX_GROUPS + 1]; };
+cudaError_t launch_group_count(const KrylovState& s, int ngroups, GroupBounds bounds, int* d_counts, cudaStream_t st, Profiler* prof);
 cudaError_t launch_krylov_init(const KrylovDims& d, const KrylovState& s, int batch, long i0 /*index of m=0*/, long n,
                                cudaStream_t st, Profiler* prof);
 cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof);

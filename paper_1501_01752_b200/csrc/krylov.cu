@@ -507,6 +507,15 @@ __global__ void __launch_bounds__(KT) refill_v0_kernel(KrylovDims d, KrylovState
     }
 }
 
+__global__ void group_count_kernel(KrylovState s, int ngroups, GroupBounds bounds, int* __restrict__ counts) {
+    const int g = blockIdx.x;   // one warp per group
+    int c = 0;
+    for (int b = bounds.b[g] + threadIdx.x; b < bounds.b[g + 1]; b += 32) c += s.active[b] != 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (threadIdx.x == 0) counts[g] = c;
+}
+
 // ---- host-side launchers ----------------------------------------------------------------------------------------
 #define GSM_E 4   // elements per thread in the sweeps (KrylovDims.chunk = KT * GSM_E)
 
@@ -586,6 +595,39 @@ cudaError_t launch_combine(const KrylovDims& d, const KrylovState& s, int batch,
                            Profiler* prof, const int* d_mask) {
     ProfScope ps_(prof, KC_COMBINE, st);   // (m_b + 1) V per solve, billed by run_batch from the iteration counts
     combine_kernel<GSM_E><<<dim3(d.nchunk, batch), KT, sizeof(cplx) * d.mmax, st>>>(d, s, batch, d_x0, d_E, d_mask);
+    return cudaGetLastError();
+}
+KrylovState krylov_state_view(const KrylovDims& d, const KrylovState& s, int b0, int* nactive) {
+    KrylovState v = s;
+    const size_t b = (size_t)b0;
+    v.basis = s.basis + b * d.vlen;
+    v.part = s.part + b * 2 * d.ld * d.nchunk;
+    v.gram = s.gram + b * d.ld * d.ld;
+    v.hcol = s.hcol + b * d.ld;
+    v.R = s.R + b * d.ld * d.mmax;
+    v.cs = s.cs + b * d.mmax;
+    v.sn = s.sn + b * d.mmax;
+    v.g = s.g + b * d.ld;
+    v.ycoef = s.ycoef + b * d.mmax;
+    v.hist = s.hist + b * d.mmax;
+    v.beta = s.beta + b;
+    v.bnorm = s.bnorm + b;
+    v.guess = s.guess + b;
+    v.rflag = s.rflag + b;
+    v.scale = s.scale + b;
+    v.active = s.active + b;
+    v.iters = s.iters + b;
+    v.nactive = nactive;
+    v.pol = s.pol + 6 * b;
+    v.running = s.running + b;
+    v.fin = s.fin + b;
+    v.point = s.point + b;
+    v.newv = s.newv + b;
+    return v;
+}
+cudaError_t launch_group_count(const KrylovState& s, int ngroups, GroupBounds bounds, int* d_counts, cudaStream_t st, Profiler* prof) {
+    ProfScope ps_(prof, KC_SMALL, st);
+    group_count_kernel<<<ngroups, 32, 0, st>>>(s, ngroups, bounds, d_counts);
     return cudaGetLastError();
 }
 cudaError_t launch_refill_mark(const KrylovDims& d, const KrylovState& s, int batch, cudaStream_t st, Profiler* prof) {
