@@ -20,7 +20,9 @@ profiling OFF.  `e2e`: per step the voxel grid is uploaded from pinned host memo
 (gsm_plan_set_cell), then the scan (through scan_shard.sharded_scan: this rank's block of the list, host-side gather),
 the device->host read of the responses, and the host pole search.  `roofline` / `kernel_ms_per_step`: a SECOND pass of
 the same K steps with every launch bracketed by CUDA events on the plan's stream (gsm_plan_profile); algorithmic bytes
-are billed from the final iteration counts of every solve.  `cpu_baseline`: the CPU oracle as it stands (O(n^2)
+are billed from the final iteration counts of every solve.  (In that pass a lock-step batch iterates as one group of
+solves; unprofiled it iterates as 2-4 groups on streams of their own, so its kernels overlap and the step is shorter
+than the sum of the kernel times.)  `cpu_baseline`: the CPU oracle as it stands (O(n^2)
 Toeplitz product + full GMRES) on one of the 256 points, plus one operator apply (the metric's other half).
 
 --impl reference: the oracle itself on the host cores, one solve (one point of the scan) per step.
@@ -522,7 +524,10 @@ def run_gsm(args):
                           "definition": "SURVEY 8(d) B_solve summed over the batch / step time (profiling off)"},
         "profiled_pass": {"ms_per_step": ms_profiled,
                           "note": "second pass of the same steps with a CUDA event pair around every launch; "
-                                  "roofline, kernel_ms_per_step and kernel_GBps come from it, value and e2e do not"},
+                                  "roofline, kernel_ms_per_step and kernel_GBps come from it, value and e2e do not. With "
+                                  "profiling on, a lock-step batch iterates as one group; without it, as 2-4 groups on "
+                                  "streams of their own whose kernels overlap, so the kernel times of this pass add up to "
+                                  "more than ms_per_step"},
         "kernel_ms_per_step": k_ms,
         "kernel_GBps": k_gbs,
         "applies_per_s": BATCH * world / (apply_ms * 1e-3),

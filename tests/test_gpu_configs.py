@@ -478,3 +478,40 @@ def test_cluster_gram_schmidt_at_32_cubed():
     assert st2 == gsm.OK and abs(it2 - iters) <= 1 and rel(E.cpu().numpy(), E2.cpu().numpy()) <= 1e-10
     two.close()
     _check_equation_rows(geo, coeffs(geo), E.cpu().numpy()[None], kb[None], np.array([TWO_PI]), pol[None], 6)
+
+
+def test_group_concurrent_iteration_is_bit_identical():
+    """A lock-step batch of 8 or more solves iterates as 2-4 groups on streams of their own (one group's Gram-Schmidt beside
+    another's apply); with per-launch profiling on it runs as one group.  Same kernels and reductions per solve: results
+    are identical bit for bit, for mixed convergence, a zero source, guesses, and a batch that stops at max_iters."""
+    geo = wl.sphere_lattice((17, 17, 17))
+    npts = 26
+    kb, kk, pol = wl.scan_points(wl.kappa_mesh(1.02, 1.30, npts), 2, 0)
+    kb[5] = [0.3, -0.2, 1.15 * TWO_PI]
+    pol[9] = 0.0
+    plan = gsm.plan_from_geometry(geo, max_iters=80, max_batch=npts)
+    Fa = torch.empty((npts, 3, 17, 17, 17), dtype=torch.complex128, device="cuda")
+    Fb = torch.zeros_like(Fa)
+    ra, ia, resa, sta = plan.scan(kb, kk, pol, tol=1e-12, fields=Fa)                 # 4 groups
+    plan.profile(True)
+    rb, ib, resb, stb = plan.scan(kb, kk, pol, tol=1e-12, fields=Fb)                 # one group
+    plan.profile(False)
+    assert sta == stb == gsm.OK and len(set(ia.tolist())) > 2 and ia[9] == 0
+    assert np.array_equal(ia, ib) and np.array_equal(ra, rb) and np.array_equal(resa, resb) and torch.equal(Fa, Fb)
+    assert np.all(resa <= 1e-10)
+    # from guesses (the fields just computed, perturbed): the groups share the apply that forms r0
+    X0 = Fa * (1.0 + 1e-4)
+    Fc, Fd = torch.empty_like(Fa), torch.empty_like(Fa)
+    rc, ic, resc, _ = plan.scan(kb, kk, pol, tol=1e-12, x0=X0, fields=Fc)
+    plan.profile(True)
+    rd, idd, resd, _ = plan.scan(kb, kk, pol, tol=1e-12, x0=X0, fields=Fd)
+    plan.profile(False)
+    assert np.array_equal(ic, idd) and np.array_equal(rc, rd) and torch.equal(Fc, Fd) and ic.max() < ia.max()
+    plan.close()
+    short = gsm.plan_from_geometry(geo, max_iters=6, max_batch=npts)
+    r1, i1, s1, st1 = short.scan(kb, kk, pol, tol=1e-12)
+    short.profile(True)
+    r2, i2, s2, st2 = short.scan(kb, kk, pol, tol=1e-12)
+    assert st1 == st2 == gsm.NOT_CONVERGED and np.array_equal(i1, i2) and np.array_equal(r1, r2) and np.array_equal(s1, s2)
+    assert np.all(np.delete(i1, 9) == 6)
+    short.close()
