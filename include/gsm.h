@@ -22,8 +22,9 @@
  *   - Coefficient layout (gsm_plan_coeffs): c[(2N1-1)][(2N2-1)][(2N3-1)], index d_a + N_a - 1.
  *   - Pointer arguments are HOST pointers unless the name starts with d_ (DEVICE pointer, 16-byte aligned, on the
  *     plan's device).  The caller owns every argument buffer; the plan owns all device scratch.
- *   - Work is enqueued on the plan's CUDA stream.  gsm_apply returns without synchronising; every other call
- *     returns after the host results it writes are valid.
+ *   - Work is enqueued on the plan's CUDA stream (solves of 8 or more points also use streams of the plan's own, forked
+ *     from and joined to that stream with events).  gsm_apply returns without synchronising; every other call returns
+ *     after the host results it writes are valid.
  *   - Errors are return codes (no exceptions, no abort, no CPU fallback).  Negative = failure, nothing valid
  *     written; positive = warning, outputs written.  gsm_last_error gives a text for the last failure.
  */
