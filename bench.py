@@ -515,6 +515,8 @@ def run_gsm(args):
                    "mean_iters_zero_start_wave": float(np.mean(iters[wave0])),
                    "mean_iters_guessed_waves": float(np.mean(iters[~wave0])) if guessed else None,
                    "max_true_resid": float(np.max(resid)), "parallelism": f"scan list sharded over {world} GPU(s), no collective",
+                   "streams": "a lock-step batch of 8+ solves iterates as 2-4 groups on streams of the plan's own "
+                              "(forked from / joined to the plan's stream); the timed region is bracketed on the plan's stream",
                    "l2": "working set per step ~24 GB >> 126 MB L2; no flush needed"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "includes": "voxel grid H2D from pinned memory + a0 (gsm_plan_set_cell) + gsm_scan + response D2H + host pole search"},
