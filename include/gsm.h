@@ -222,7 +222,42 @@ gsm_status gsm_retrieve_neff_many(gsm_plan* plan, int nlines, const double* dir,
                                   const double* k0, const double* n_lo, const double* n_hi, int ncoarse, int nfine,
                                   double fine_step, double tol, double* out, int* line_status);
 
-/* Text of the last failure on this plan (or of the last failed gsm_plan_create when plan == NULL). */
+/* ---- Operator apply for callers that cannot allocate -------------------------------------------------------------------
+ * gsm_apply_static computes the same y[b] = x[b] - G(k_bloch[b], k0[b]) (T x[b]) as gsm_apply (Eq. 4; with
+ * formulation = GSM_FORM_H the operator of Eq. 5), but takes no plan and calls no cudaMalloc, cudaFree,
+ * cudaMallocHost or other allocating routine - not on the first call either.
+ *
+ * Who needs it: gsm_plan_create takes all of a plan's memory from cudaMalloc.  A program that embeds this library may be
+ * unable to do that - its own allocator (a deep-learning framework's caching allocator, a server's pre-reserved pool)
+ * already owns the device memory so that a further cudaMalloc fails or escapes its accounting, it runs under a per-client
+ * memory quota, or it sits in a latency-bound loop where the device-wide synchronisation of cudaMalloc / cudaFree is not
+ * acceptable.  Such a caller passes buffers from its own allocator for the inputs and the output; the intermediates
+ * (transformed coefficient grid, z-transformed field) go to a fixed array of GSM_STATIC_SCRATCH_BYTES that is part of the
+ * library image: every GPU that loads the library carries those bytes until the process exits, used or not.
+ *
+ * Limits (the price of a fixed array): orders[a] <= GSM_STATIC_MAX_ORDER per axis, batch <= GSM_STATIC_MAX_BATCH.  Anything
+ * larger is refused with GSM_E_INVALID and a text from gsm_last_error(NULL) that names the limit; nothing is written.
+ *
+ * Arguments: period[3], orders[3], eps_b, formulation as in gsm_plan_desc.  d_coef: DEVICE, the Toeplitz generator c_d
+ * ((2N1-1)(2N2-1)(2N3-1) complex, the layout of gsm_plan_coeffs; D_d for GSM_FORM_H), read on every call - the spectrum is
+ * rebuilt each time since there is no plan to keep it.  k_bloch[batch][3], k0[batch]: HOST, copied before return.
+ * d_x, d_y: DEVICE, [batch][3][N1][N2][N3] complex, 16-byte aligned, not overlapping.  cuda_stream: cudaStream_t to enqueue
+ * on (NULL = legacy default stream).  All device pointers belong to the CURRENT device.  Asynchronous like gsm_apply.
+ *
+ * First call on a device: looks up the array's device address, sets kernel attributes and copies 1 KiB of FFT twiddles
+ * into it with a synchronous cudaMemcpy.  Make that first call outside any stream capture.
+ *
+ * Sharing: there is ONE array per device.  Every call on that device uses it, and it keeps the previous call's contents;
+ * the entry point clears or fully overwrites whatever it later reads, so stale contents never matter.  Calls that overlap
+ * on the GPU (two streams, two host threads) race on the array and give wrong results - the caller must serialise them. */
+#define GSM_STATIC_MAX_ORDER 16
+#define GSM_STATIC_MAX_BATCH 4
+#define GSM_STATIC_SCRATCH_BYTES 2622720
+gsm_status gsm_apply_static(const double period[3], const int orders[3], double eps_b_re, double eps_b_im, int formulation,
+                            const void* d_coef, int batch, const double* k_bloch, const double* k0, const void* d_x,
+                            void* d_y, void* cuda_stream);
+
+/* Text of the last failure on this plan (or, when plan == NULL, of the last failed gsm_plan_create or gsm_apply_static). */
 const char* gsm_last_error(const gsm_plan* plan);
 
 #ifdef __cplusplus

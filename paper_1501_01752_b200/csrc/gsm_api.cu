@@ -574,6 +574,21 @@ extern "C" gsm_status gsm_apply(gsm_plan* plan, int batch, const double* k_bloch
     return GSM_OK;
 }
 
+// Plan-free, allocation-free operator apply (apply_static.cu); the failure text goes where gsm_last_error(NULL) finds it.
+namespace gsm {
+gsm_status apply_static(const double period[3], const int orders[3], double eps_b_re, double eps_b_im, int formulation,
+                        const void* d_coef, int batch, const double* k_bloch, const double* k0, const void* d_x, void* d_y,
+                        cudaStream_t st, std::string* err);
+}
+extern "C" gsm_status gsm_apply_static(const double period[3], const int orders[3], double eps_b_re, double eps_b_im,
+                                       int formulation, const void* d_coef, int batch, const double* k_bloch,
+                                       const double* k0, const void* d_x, void* d_y, void* cuda_stream) {
+    std::string msg;
+    const gsm_status st = gsm::apply_static(period, orders, eps_b_re, eps_b_im, formulation, d_coef, batch, k_bloch, k0, d_x,
+                                            d_y, static_cast<cudaStream_t>(cuda_stream), &msg);
+    return st < 0 ? fail(nullptr, st, msg.c_str()) : st;
+}
+
 // nb <= max_batch solves in lock step.  d_E: device [nb][vlen].  d_x0 (may be null, may alias d_E): initial guesses.
 // Host outputs may be null.
 static gsm_status run_batch(gsm_plan* plan, int nb, const double* kvec, const double* k0, const double* pol, double tol,

@@ -20,6 +20,7 @@ SPHERE, ELLIPSOID, BOX, POLYHEDRON = 0, 1, 2, 3
 FORM_E, FORM_H = 0, 1
 FLAG_TWO_SWEEP, FLAG_GENERIC_APPLY, FLAG_FUSED_APPLY, FLAG_SLOT_REFILL = 1, 2, 4, 8   # include/gsm.h GSM_FLAG_*
 MAX_ITERS = 512
+STATIC_MAX_ORDER, STATIC_MAX_BATCH, STATIC_SCRATCH_BYTES = 16, 4, 2622720   # include/gsm.h GSM_STATIC_*
 
 
 class GsmError(RuntimeError):
@@ -79,6 +80,8 @@ def _load():
     lib.gsm_retrieve_neff.restype = C.c_int
     lib.gsm_retrieve_neff_many.argtypes = [P, C.c_int, P, P, P, P, P, P, C.c_int, C.c_int, C.c_double, C.c_double, P, P]
     lib.gsm_retrieve_neff_many.restype = C.c_int
+    lib.gsm_apply_static.argtypes = [P, P, C.c_double, C.c_double, C.c_int, P, C.c_int, P, P, P, P, P]
+    lib.gsm_apply_static.restype = C.c_int
     lib.gsm_last_error.argtypes = [P]
     lib.gsm_last_error.restype = C.c_char_p
     for f in ("gsm_plan_create", "gsm_plan_destroy", "gsm_plan_coeffs", "gsm_plan_info", "gsm_apply", "gsm_solve",
@@ -317,6 +320,32 @@ class Plan:
         if st < 0 and not np.any(ls == OK):
             _check(st, self._h)
         return out[:, 0] + 1j * out[:, 1], out[:, 2] + 1j * out[:, 3], out[:, 4] + 1j * out[:, 5], ls, st
+
+
+def apply_static(periods, orders, eps_b, coef, k_bloch, k0, x, out, formulation=FORM_E, stream=None):
+    """gsm_apply_static: y = x - G (T x) without a plan, for programs that must not touch the CUDA allocator.
+
+    Meant for hosts whose own allocator already owns the GPU's memory (or that run under a memory quota, or cannot
+    afford cudaMalloc's device-wide synchronisation): the library allocates nothing here, its intermediates live in a
+    fixed STATIC_SCRATCH_BYTES array inside the library image.  In the same spirit this wrapper allocates nothing on the
+    device either - `out` is required.  coef: cuda complex128 tensor [2N1-1, 2N2-1, 2N3-1] (layout of Plan.coeffs());
+    x, out: cuda complex128 [batch, 3, N1, N2, N3], distinct; orders <= STATIC_MAX_ORDER per axis, batch <=
+    STATIC_MAX_BATCH (larger sizes raise GsmError naming the limit).  Enqueued on `stream` (default: torch's current
+    stream).  One scratch array per GPU is shared by all calls: do not let two calls overlap on the device."""
+    import torch
+    orders = tuple(int(n) for n in orders)
+    batch = int(x.shape[0])
+    for t in (coef, x, out):
+        assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()
+    assert tuple(coef.shape) == tuple(2 * n - 1 for n in orders)
+    assert tuple(x.shape) == (batch, 3) + orders and tuple(out.shape) == tuple(x.shape)
+    per = _f64(periods, (3,))
+    od = np.ascontiguousarray(orders, dtype=np.int32)
+    kb, kk = _f64(k_bloch, (batch, 3)), _f64(k0, (batch,))
+    st = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+    _check(_lib.gsm_apply_static(per.ctypes.data, od.ctypes.data, complex(eps_b).real, complex(eps_b).imag, int(formulation),
+                                 coef.data_ptr(), batch, kb.ctypes.data, kk.ctypes.data, x.data_ptr(), out.data_ptr(), st))
+    return out
 
 
 def mesh_schedule(npts, levels, collapse_after=0):
