@@ -322,7 +322,8 @@ def gmres(apply, b: np.ndarray, tol: float, max_iters: int, x0: np.ndarray | Non
     with a non-zero initial guess).  The stop test stays relative to ||b||, so every start meets the same bar.
 
     Returns (x, history, iters): history[j] = |g_{j+1}| / ||b|| after iteration j+1.
-    Lucky breakdown (h_{j+1,j} = 0) exits as converged (reading R23).
+    Lucky breakdown (h_{j+1,j} <= eps ||A v_j||: nothing of A v_j is left after orthogonalisation) exits as converged
+    (reading R23; the test is scale-free, so it acts the same for a guessed start with a tiny ||r0||).
     """
     shape = b.shape
     bv = b.ravel()
@@ -353,6 +354,7 @@ def gmres(apply, b: np.ndarray, tol: float, max_iters: int, x0: np.ndarray | Non
             w -= H[i, j] * V[i]
         hn = np.linalg.norm(w)
         H[j + 1, j] = hn
+        wnorm = np.linalg.norm(H[: j + 2, j])                    # ||A v_j|| (Pythagoras over v_0..v_j and the remainder)
         for i in range(j):                                       # previous rotations on the new column
             t = cs[i] * H[i, j] + sn[i] * H[i + 1, j]
             H[i + 1, j] = -np.conj(sn[i]) * H[i, j] + cs[i] * H[i + 1, j]
@@ -372,7 +374,7 @@ def gmres(apply, b: np.ndarray, tol: float, max_iters: int, x0: np.ndarray | Non
         g[j] = cs[j] * g[j]
         m = j + 1
         hist.append(abs(g[j + 1]) / bnorm)
-        if hist[-1] <= tol or hn <= np.finfo(float).eps * beta:
+        if hist[-1] <= tol or hn <= np.finfo(float).eps * wnorm:
             break
         V.append(w / hn)
     y = np.zeros(m, dtype=np.complex128)

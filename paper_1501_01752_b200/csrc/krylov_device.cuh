@@ -14,8 +14,10 @@ __device__ __forceinline__ void givens_step(const KrylovDims& d, const KrylovSta
     cplx* sn = s.sn + (long)b * d.mmax;
     cplx* g = s.g + (long)b * d.ld;
     cplx hi = h[0];
+    double col2 = hi.x * hi.x + hi.y * hi.y + hn * hn;   // ||(h_0j .. h_jj, h_{j+1,j})||^2 = ||A v_j||^2 up to rounding
     for (int i = 0; i < j; ++i) {   // previous rotations on the new column
         const cplx hn1 = h[i + 1];
+        col2 += hn1.x * hn1.x + hn1.y * hn1.y;
         const double ci = cs_prev[i];
         const cplx si = sn_prev[i];
         const cplx t = cadd(make_double2(ci * hi.x, ci * hi.y), cmul(si, hn1));
@@ -38,11 +40,12 @@ __device__ __forceinline__ void givens_step(const KrylovDims& d, const KrylovSta
     const cplx gn = make_double2(-(sv.x * gj.x + sv.y * gj.y), -(sv.x * gj.y - sv.y * gj.x));   // -conj(sn) g_j
     g[j + 1] = gn;
     g[j] = make_double2(c * gj.x, c * gj.y);
-    const double beta = s.beta[b];
     const double res = hypot(gn.x, gn.y) / s.bnorm[b];
     s.hist[(long)b * d.mmax + j] = res;
     s.iters[b] = j + 1;
-    const bool lucky = hn <= 2.220446049250313e-16 * beta;
+    // reading R23: the new direction has vanished relative to the vector it was orthogonalised from.  Scale-free, so a
+    // solve started from a guess (||r0|| tiny against ||b||) is guarded exactly like a zero start.
+    const bool lucky = hn <= 2.220446049250313e-16 * sqrt(col2);
     if (res <= s.tol[0] || lucky) {
         s.active[b] = 0;
         atomicSub(s.nactive, 1);

@@ -62,6 +62,29 @@ def test_homogeneous_cell_lucky_breakdown():
     plan.close()
 
 
+def test_guessed_start_near_breakdown_stays_finite():
+    """Reading R23 with a guessed start (oracle pin: test_gmres_guess_off_by_one_eigenvector_...): x0 = x* + 1e-7 u with u
+    an eigenvector of A, and a tolerance that cannot be met.  After one iteration nothing but rounding is left of A v_0;
+    whether the device calls that a breakdown (h_10 <= eps ||A v_0||) or keeps orthogonalising rounding noise, the
+    returned field must be the exact solution, finite, with a true residual at rounding level."""
+    geo = wl.Geometry("uniform", (0.2, 0.2, 0.2), (3, 3, 3),
+                      [dict(kind=wl.BOX, center=(0, 0, 0), size=(0.2, 0.2, 0.2), eps=2.5)], 1.0, 1.0, None, ())
+    c = orc.coeffs_analytic(geo.periods, geo.orders, geo.shapes, geo.eps_bg, geo.eps_b)
+    kb = np.array([[0.0, 0.0, 1.3 * TWO_PI]])
+    ref = orc.solve_dense(c, geo.periods, geo.orders, kb[0], TWO_PI, geo.eps_b, [1.0, 0, 0])
+    u = np.zeros_like(ref)
+    u[1, 2, 1, 1] = 1.0
+    plan = gsm.plan_from_geometry(geo, max_iters=20)
+    fields = torch.empty((1, 3, 3, 3, 3), dtype=torch.complex128, device="cuda")
+    x0 = torch.from_numpy((ref + 1e-7 * u)[None]).cuda()
+    resp, iters, resid, st = plan.scan(kb, [TWO_PI], np.array([[1.0, 0, 0, 0, 0, 0]]), tol=1e-30, fields=fields, x0=x0)
+    E = fields.cpu().numpy()[0]
+    assert st in (gsm.OK, gsm.NOT_CONVERGED) and 1 <= iters[0] <= 20
+    assert np.all(np.isfinite(E.view(np.float64))) and np.isfinite(resid[0]) and resid[0] <= 1e-14
+    assert np.linalg.norm(E - ref) / np.linalg.norm(ref) <= 1e-13
+    plan.close()
+
+
 def test_uniform_cell_closed_form():
     """c_d = Delta delta_d0: E_0 = a (kappa^2 - k0^2 eps_b)/(kappa^2 - k0^2 eps_2) for transverse a."""
     eps2, eps_b = 2.5, 1.0

@@ -469,3 +469,23 @@ def test_polyhedron_coefficients_vs_voxelised_direct_dft():
             inside &= (r @ n) <= o
         errs.append(np.abs(O.coeffs_voxel(np.where(inside, sh["eps"], 1.0), g.orders, 1.0) - c).max())
     assert errs[0] > errs[1] > errs[2] and errs[2] < 1e-2 * abs(c[2, 2, 2])
+
+
+def test_gmres_guess_off_by_one_eigenvector_breaks_down_after_one_iteration():
+    """Reading R23 with a guessed start.  Uniform cell: A is block diagonal over the harmonics and a unit vector u at
+    harmonic m = (1, 0, 0) polarised along y (transverse to k_m) is an eigenvector.  x0 = x* + 1e-7 u gives r0 parallel
+    to u, so the Krylov space is one-dimensional: A v_0 has nothing left after orthogonalisation and GMRES must stop
+    after ONE iteration at the exact solution, even with a tolerance that can never be met.  ||r0|| is 1e-7 ||b|| here:
+    a breakdown test scaled by ||r0|| would miss it and go on dividing by a rounding-level h_{j+1,j}."""
+    eps2 = 2.5
+    g = W.Geometry("uniform", (0.2, 0.2, 0.2), (3, 3, 3),
+                   [dict(kind=W.BOX, center=(0, 0, 0), size=(0.2, 0.2, 0.2), eps=eps2)], 1.0, 1.0, None, ())
+    c = coeffs(g)
+    kb, pol = np.array([0.0, 0.0, 1.3 * K0]), [1.0, 0.0, 0.0]
+    ref = O.solve_dense(c, g.periods, g.orders, kb, K0, 1.0, pol)
+    u = np.zeros_like(ref)
+    u[1, 2, 1, 1] = 1.0                                   # component y at m = (+1, 0, 0)
+    lam = (O.apply_operator(c, u, g.periods, kb, K0, 1.0))[1, 2, 1, 1]
+    assert np.linalg.norm(O.apply_operator(c, u, g.periods, kb, K0, 1.0) - lam * u) < 1e-14      # u is an eigenvector
+    E, h, m = O.solve_gmres(c, g.periods, g.orders, kb, K0, 1.0, pol, tol=1e-30, max_iters=20, x0=ref + 1e-7 * u)
+    assert m == 1 and np.linalg.norm(E - ref) / np.linalg.norm(ref) < 1e-14
