@@ -220,6 +220,25 @@ class Plan:
         return {"fft_grid": tuple(g), "device_bytes": b.value, "launches": l.value}
 
     # -- hot path -------------------------------------------------------------------------------------------
+    def _order_before(self):
+        """Plan bound to a side stream: make it wait for the work already queued on torch's current stream (which may
+        still be producing the tensors handed in).  Returns the current stream, or None when no ordering is needed."""
+        cur = self._torch.cuda.current_stream()
+        if self.stream is None or self.stream == cur:
+            return None
+        self.stream.wait_stream(cur)
+        return cur
+
+    def _order_after(self, cur, *tensors):
+        """Counterpart of _order_before: the current stream waits for the plan's stream, and the caching allocator is
+        told that the plan's stream used `tensors` (so their memory is not recycled under it)."""
+        if cur is None:
+            return
+        cur.wait_stream(self.stream)
+        for t in tensors:
+            if t is not None:
+                t.record_stream(self.stream)
+
     def apply(self, k_bloch, k0, x, out=None):
         """gsm_apply: y = x - G (T x).  x: cuda complex128 tensor [batch, 3, N1, N2, N3].
 
@@ -230,27 +249,28 @@ class Plan:
         assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous() and tuple(x.shape[1:]) == (3,) + self.orders
         y = torch.empty_like(x) if out is None else out
         kb, kk = _f64(k_bloch, (batch, 3)), _f64(k0, (batch,))
-        cur = torch.cuda.current_stream()
-        side = self.stream is not None and self.stream != cur
-        if side:
-            self.stream.wait_stream(cur)
-        _check(_lib.gsm_apply(self._h, batch, kb.ctypes.data, kk.ctypes.data, x.data_ptr(), y.data_ptr()), self._h)
-        if side:
-            cur.wait_stream(self.stream)
-            x.record_stream(self.stream)
-            y.record_stream(self.stream)
+        cur = self._order_before()
+        try:
+            _check(_lib.gsm_apply(self._h, batch, kb.ctypes.data, kk.ctypes.data, x.data_ptr(), y.data_ptr()), self._h)
+        finally:
+            self._order_after(cur, x, y)
         return y
 
     def solve(self, k_bloch, k0, pol, tol=1e-10, out=None):
-        """gsm_solve: returns (E cuda tensor [3,N1,N2,N3], residual history, iterations, true residual, status)."""
+        """gsm_solve: returns (E cuda tensor [3,N1,N2,N3], residual history, iterations, true residual, status).
+        Ordered against torch's current stream like apply()."""
         torch = self._torch
         E = torch.empty((3,) + self.orders, dtype=torch.complex128, device="cuda") if out is None else out
         kb = _f64(k_bloch, (3,))
         pl = _f64(np.asarray(pol, dtype=np.complex128).view(np.float64), (6,))
         hist = np.zeros(self.max_iters)
         it, res = C.c_int(), C.c_double()
-        st = _check(_lib.gsm_solve(self._h, kb.ctypes.data, float(k0), pl.ctypes.data, float(tol), E.data_ptr(),
-                                   hist.ctypes.data, self.max_iters, C.byref(it), C.byref(res)), self._h)
+        cur = self._order_before()
+        try:
+            st = _check(_lib.gsm_solve(self._h, kb.ctypes.data, float(k0), pl.ctypes.data, float(tol), E.data_ptr(),
+                                       hist.ctypes.data, self.max_iters, C.byref(it), C.byref(res)), self._h)
+        finally:
+            self._order_after(cur, E)
         return E, hist[: it.value].copy(), it.value, res.value, st
 
     def history(self, b=0):
@@ -266,7 +286,9 @@ class Plan:
         pol: [npts, 6] real (interleaved complex) or [npts, 3] complex.  fields: optional cuda tensor
         [npts, 3, N1, N2, N3] that receives every solution.  x0: optional cuda tensor of the same shape with initial
         guesses (gsm_scan_guess; may be `fields` itself).  levels: solve the list as an ordered equidistant mesh in
-        that many coarse-to-fine waves, each started from the interpolation of the previous ones (gsm_scan_mesh)."""
+        that many coarse-to-fine waves, each started from the interpolation of the previous ones (gsm_scan_mesh).
+        With the plan on a side stream the call is ordered after torch's current stream (which may still be writing x0)
+        and the current stream after the call (which may read fields), like apply()."""
         kb = _f64(k_bloch)
         npts = kb.shape[0]
         kk = _f64(k0, (npts,))
@@ -278,6 +300,14 @@ class Plan:
         iters = np.zeros(npts, dtype=np.int32)
         resid = np.zeros(npts)
         fp = fields.data_ptr() if fields is not None else None
+        cur = self._order_before()
+        try:
+            st = self._scan_call(npts, kb, kk, pl, tol, levels, x0, resp, iters, resid, fp)
+        finally:
+            self._order_after(cur, x0, fields)
+        return resp, iters, resid, _check(st, self._h)
+
+    def _scan_call(self, npts, kb, kk, pl, tol, levels, x0, resp, iters, resid, fp):
         if levels is not None:
             assert x0 is None
             st = _lib.gsm_scan_mesh(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol), int(levels),
@@ -289,7 +319,7 @@ class Plan:
         else:
             st = _lib.gsm_scan(self._h, npts, kb.ctypes.data, kk.ctypes.data, pl.ctypes.data, float(tol),
                                resp.ctypes.data, iters.ctypes.data, resid.ctypes.data, fp)
-        return resp, iters, resid, _check(st, self._h)
+        return st
 
 
     def retrieve_neff(self, direction, pol, comp, k0, n_lo, n_hi, ncoarse=29, nfine=18, fine_step=0.002, tol=1e-10):

@@ -270,6 +270,35 @@ def test_fused_apply_many_solves_ring_reuse_and_inactive_solves():
 
 
 # ---- Krylov work reused along the kappa mesh --------------------------------------------
+def test_scan_guess_on_a_side_stream_is_ordered_with_the_current_stream():
+    """Plan.scan / Plan.solve on a plan bound to its own stream: the guesses x0 are produced by a chain of kernels on
+    torch's current stream right before the call and the fields are read on it right after, with no manual
+    synchronisation.  Same results, bit for bit, as a plan on the current stream."""
+    geo = wl.sphere_lattice((17, 17, 17))
+    kappa = np.array([1.12, 1.13, 1.14, 1.15]) * TWO_PI
+    kb, kk, pol = wl.scan_points(kappa, 2, 0)
+    side = torch.cuda.Stream()
+    p_side = gsm.plan_from_geometry(geo, max_iters=64, max_batch=4, stream=side)
+    p_ref = gsm.plan_from_geometry(geo, max_iters=64, max_batch=4)
+    base = torch.empty((4, 3, 17, 17, 17), dtype=torch.complex128, device="cuda")
+    p_ref.scan(kb * (1 + 5e-4), kk, pol, tol=1e-10, fields=base)          # neighbouring points' fields as guesses
+    torch.cuda.synchronize()
+    for rep in range(3):
+        x0 = base * 0.0
+        for _ in range(20):                       # a chain of kernels on the current stream that produces x0
+            x0 = x0 + base / 20.0
+        f_side = torch.empty_like(base)
+        r1, i1, _, _ = p_side.scan(kb, kk, pol, tol=1e-10, fields=f_side, x0=x0)
+        got = f_side.cpu().numpy()                # read on the current stream
+        f_ref = torch.empty_like(base)
+        r2, i2, _, _ = p_ref.scan(kb, kk, pol, tol=1e-10, fields=f_ref, x0=x0)
+        assert np.array_equal(i1, i2) and np.array_equal(r1, r2) and np.array_equal(got, f_ref.cpu().numpy())
+        E1 = p_side.solve(kb[0], TWO_PI, [1.0, 0, 0], tol=1e-10)[0].cpu().numpy()
+        E2 = p_ref.solve(kb[0], TWO_PI, [1.0, 0, 0], tol=1e-10)[0].cpu().numpy()
+        assert np.array_equal(E1, E2)
+    p_side.close(); p_ref.close()
+
+
 def test_scan_guess_matches_oracle_gmres_with_the_same_x0():
     """gsm_scan_guess: GMRES from an initial guess (r0 = b - A x0, E = x0 + d) against the oracle's gmres(x0=...) with the
     SAME x0: the solution of a nearby kappa point, a random field (worse than a zero start: the library falls back to
