@@ -4,7 +4,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <new>
+#include <utility>
 
 #include "gsm_internal.cuh"
 
@@ -82,6 +84,17 @@ static cudaError_t dalloc(gsm_plan* p, T** out, size_t count) {
     return cudaSuccess;
 }
 
+// Give back one block obtained from dalloc (used where a workspace is replaced by one of another size).
+template <typename T>
+static void dfree(gsm_plan* p, T** ptr, size_t count) {
+    if (!*ptr) return;
+    auto it = std::find(p->allocs.begin(), p->allocs.end(), static_cast<void*>(*ptr));
+    if (it != p->allocs.end()) p->allocs.erase(it);
+    cudaFree(*ptr);
+    p->device_bytes -= (long long)(std::max<size_t>(count, 1) * sizeof(T));
+    *ptr = nullptr;
+}
+
 static int fft_size(int N) {
     if (N == 1) return 1;
     int p = 1;
@@ -146,19 +159,28 @@ static cplx cdivh(double ar, double ai, double br, double bi) {
     return make_double2((ar * br + ai * bi) * inv, (ai * br - ar * bi) * inv);
 }
 
-// Polyhedron geometry for the device (plan_kernels.cu polyhedron_image): normals, areas, edges.  False if the
-// description is malformed (index out of range, degenerate face, fewer than 4 faces).
-static bool prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<PolyFace>& faces, std::vector<PolyEdge>& edges) {
-    if (s.n_vertices < 4 || s.n_faces < 4 || !s.vertices || !s.face_sizes || !s.face_vertices) return false;
+// Polyhedron geometry for the device (plan_kernels.cu polyhedron_image): normals, areas, edges.  Returns null, or the
+// reason the description is malformed: index out of range, degenerate or non-planar face, fewer than 4 faces, a surface
+// that is not closed and consistently oriented (every directed edge a -> b of a face must be matched by exactly one
+// b -> a of another face: one face listed clockwise, a missing face or a doubled face all break this), or inward
+// orientation as a whole (negative volume).  The closed form of reading R27 is only valid for such a surface.
+static const char* prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<PolyFace>& faces, std::vector<PolyEdge>& edges) {
+    if (s.n_vertices < 4 || s.n_faces < 4 || !s.vertices || !s.face_sizes || !s.face_vertices)
+        return "polyhedron needs at least 4 vertices and 4 faces";
+    std::map<std::pair<int, int>, int> directed;   // directed edge -> how often it occurs
     q.f0 = (int)faces.size();
     q.nf = s.n_faces;
     q.vol = 0.0;
     const int* fv = s.face_vertices;
     for (int f = 0; f < s.n_faces; ++f) {
         const int cnt = s.face_sizes[f];
-        if (cnt < 3) return false;
+        if (cnt < 3) return "polyhedron face with fewer than 3 vertices";
         for (int k = 0; k < cnt; ++k)
-            if (fv[k] < 0 || fv[k] >= s.n_vertices) return false;
+            if (fv[k] < 0 || fv[k] >= s.n_vertices) return "polyhedron vertex index out of range";
+        for (int k = 0; k < cnt; ++k) {
+            const int a = fv[k], b = fv[(k + 1) % cnt];
+            if (a == b || ++directed[std::make_pair(a, b)] > 1) return "polyhedron surface is not closed and consistently oriented (repeated edge)";
+        }
         auto V = [&](int k) { return s.vertices + 3 * (size_t)fv[k % cnt]; };
         PolyFace F{};
         double nv[3] = {0.0, 0.0, 0.0};
@@ -170,8 +192,12 @@ static bool prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<Poly
             nv[2] += 0.5 * (a[0] * b[1] - a[1] * b[0]);
         }
         F.area = std::sqrt(nv[0] * nv[0] + nv[1] * nv[1] + nv[2] * nv[2]);
-        if (!(F.area > 0.0)) return false;
+        if (!(F.area > 0.0)) return "degenerate polyhedron face (zero area)";
         for (int a = 0; a < 3; ++a) { F.n[a] = nv[a] / F.area; F.p0[a] = V(0)[a]; }
+        for (int k = 1; k < cnt; ++k) {               // planarity: distance of every vertex from the plane through V(0)
+            const double dist = (V(k)[0] - F.p0[0]) * F.n[0] + (V(k)[1] - F.p0[1]) * F.n[1] + (V(k)[2] - F.p0[2]) * F.n[2];
+            if (std::fabs(dist) > 1e-9 * std::sqrt(F.area)) return "polyhedron face is not planar";
+        }
         q.vol += (F.p0[0] * F.n[0] + F.p0[1] * F.n[1] + F.p0[2] * F.n[2]) * F.area / 3.0;
         F.e0 = (int)edges.size();
         F.ne = cnt;
@@ -192,7 +218,10 @@ static bool prepare_polyhedron(const gsm_shape& s, ShapeDev& q, std::vector<Poly
         faces.push_back(F);
         fv += cnt;
     }
-    return q.vol > 0.0;
+    for (const auto& kv : directed)
+        if (!directed.count(std::make_pair(kv.first.second, kv.first.first)))
+            return "polyhedron surface is not closed and consistently oriented (an edge without its reverse: open surface or a face listed clockwise)";
+    return q.vol > 0.0 ? nullptr : "polyhedron faces are oriented inwards (list them counter-clockwise seen from outside)";
 }
 
 // voxel grid sizes: at least the 2N - 1 harmonics needed per axis (1 is allowed for an axis with one order)
@@ -230,8 +259,7 @@ static gsm_status build_coeffs(gsm_plan* plan) {
             else if (s.kind == GSM_BOX) q.f = s.size[0] * s.size[1] * s.size[2] / vol;
             else if (s.kind == GSM_POLYHEDRON) {
                 q.f = 1.0 / vol;
-                if (!prepare_polyhedron(s, q, pfaces, pedges))
-                    return fail(plan, GSM_E_INVALID, "malformed polyhedron (indices, degenerate face, or inward orientation)");
+                if (const char* why = prepare_polyhedron(s, q, pfaces, pedges)) return fail(plan, GSM_E_INVALID, why);
             } else return fail(plan, GSM_E_INVALID, "unknown shape kind");
         }
         ShapeDev* dsh = nullptr;
@@ -268,7 +296,13 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     if (!pow2) {   // any other size: the defining sums, axis by axis, each pass keeping only the wanted harmonics
         const size_t nv = (size_t)V[0] * V[1] * V[2];
         const size_t n1 = (size_t)V[0] * V[1] * (2 * N[2] - 1), n2 = (size_t)V[0] * (2 * N[1] - 1) * (2 * N[2] - 1);
-        if (!plan->vgrid || plan->vgrid_count != nv + n1 + n2) { CK(dalloc(plan, &plan->vgrid, nv + n1 + n2)); plan->vgrid_count = nv + n1 + n2; }
+        if (!plan->vgrid || plan->vgrid_count != nv + n1 + n2) {   // a grid of another size replaces the old block
+            CK(cudaStreamSynchronize(plan->stream));
+            dfree(plan, &plan->vgrid, plan->vgrid_count);
+            plan->vgrid_count = 0;
+            CK(dalloc(plan, &plan->vgrid, nv + n1 + n2));
+            plan->vgrid_count = nv + n1 + n2;
+        }
         cplx *grid = plan->vgrid, *t1 = grid + nv, *t2 = t1 + n1;
         cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
         ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
@@ -292,7 +326,13 @@ static gsm_status build_coeffs(gsm_plan* plan) {
     const cplx* const* vtw = plan->vtw;
     int* const* dpos = plan->vpos;
     const size_t nv = (size_t)V[0] * V[1] * V[2];
-    if (!plan->vgrid || plan->vgrid_count != nv) { CK(dalloc(plan, &plan->vgrid, nv)); plan->vgrid_count = nv; }
+    if (!plan->vgrid || plan->vgrid_count != nv) {
+        CK(cudaStreamSynchronize(plan->stream));
+        dfree(plan, &plan->vgrid, plan->vgrid_count);
+        plan->vgrid_count = 0;
+        CK(dalloc(plan, &plan->vgrid, nv));
+        plan->vgrid_count = nv;
+    }
     cplx* grid = plan->vgrid;
     cudaError_t e = cudaMemcpyAsync(grid, d.eps_grid_host, sizeof(cplx) * nv, cudaMemcpyHostToDevice, plan->stream);
     ProfScope ps_(&plan->prof, KC_PLAN, plan->stream);
@@ -744,10 +784,12 @@ static gsm_status run_refill(gsm_plan* plan, int npts, const double* kvec, const
     const size_t per_pt = sizeof(double) * 17 + sizeof(int) * 2;
     if (plan->refill_cap < (size_t)npts) {
         if (plan->refill_buf) cudaFree(plan->refill_buf);
+        plan->device_bytes -= (long long)(per_pt * plan->refill_cap);
         plan->refill_buf = nullptr;
         plan->refill_cap = 0;
         CK(cudaMalloc(&plan->refill_buf, per_pt * (size_t)npts));
         plan->refill_cap = (size_t)npts;
+        plan->device_bytes += (long long)(per_pt * plan->refill_cap);
     }
     double* dd = static_cast<double*>(plan->refill_buf);
     cplx* d_resp = reinterpret_cast<cplx*>(dd);   // first: 16-byte aligned for any npts
@@ -946,10 +988,12 @@ extern "C" gsm_status gsm_scan_mesh(gsm_plan* plan, int npts, const double* k_bl
     if (!all) {
         if (plan->mesh_cap < (size_t)npts) {
             if (plan->mesh_fields) cudaFree(plan->mesh_fields);
+            plan->device_bytes -= (long long)(sizeof(cplx) * vlen * plan->mesh_cap);
             plan->mesh_fields = nullptr;
             plan->mesh_cap = 0;
             CK(cudaMalloc(reinterpret_cast<void**>(&plan->mesh_fields), sizeof(cplx) * vlen * npts));
             plan->mesh_cap = (size_t)npts;
+            plan->device_bytes += (long long)(sizeof(cplx) * vlen * plan->mesh_cap);
         }
         all = plan->mesh_fields;
     }

@@ -58,8 +58,9 @@ def test_coeffs_analytic(geo):
 
 
 def test_polyhedron_rejects_malformed_descriptions_and_solves_vs_dense_lu():
-    """GSM_POLYHEDRON (PAPER.md:62, :99): inward-oriented faces, a bad vertex index and a two-vertex face are rejected;
-    a lattice of rotated cubes is solved against the oracle's dense LU."""
+    """GSM_POLYHEDRON: inward-oriented faces, a bad vertex index, a two-vertex face, a single flipped
+    face, an open surface, a doubled face and a non-planar face are rejected; a lattice of rotated cubes is solved against
+    the oracle's dense LU."""
     geo = wl.polyhedron_lattice((5, 5, 5), "cube", scale=0.05, eps=9.0)
     sh = geo.shapes[0]
     for bad in (dict(sh, faces=[tuple(reversed(f)) for f in sh["faces"]]),
@@ -68,6 +69,17 @@ def test_polyhedron_rejects_malformed_descriptions_and_solves_vs_dense_lu():
         with pytest.raises(gsm.GsmError) as e:
             gsm.Plan(geo.periods, geo.orders, shapes=[bad])
         assert e.value.status == gsm.E_INVALID
+    # a surface that is not closed and consistently oriented would pass a volume-sign test and give wrong harmonics
+    faces = list(sh["faces"])
+    bent = np.array(sh["vertices"], dtype=float).copy()
+    bent[0] += 1e-3 * (bent[0] - bent[7])                       # pull one corner of the cube outwards: three bent quads
+    for bad, word in ((dict(sh, faces=[tuple(reversed(faces[0]))] + faces[1:]), "closed"),      # one face clockwise
+                      (dict(sh, faces=faces[:-1]), "closed"),                                   # open: a face missing
+                      (dict(sh, faces=faces + [faces[2]]), "closed"),                           # a face listed twice
+                      (dict(sh, vertices=bent), "planar")):
+        with pytest.raises(gsm.GsmError) as e:
+            gsm.Plan(geo.periods, geo.orders, shapes=[bad])
+        assert e.value.status == gsm.E_INVALID and word in str(e.value)
     plan = gsm.plan_from_geometry(geo, max_iters=80)
     kb, pol = np.array([0.2, -0.1, 1.2 * TWO_PI]), np.array([1.0, 0.3j, 0.0])
     E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
@@ -284,6 +296,16 @@ def test_set_cell_rebuilds_harmonics_in_place():
     y = plan.apply(kb, k0, torch.from_numpy(x).cuda()).cpu().numpy()[0]
     assert rel(y, orc.apply_operator(oracle_coeffs(g3), x[0], g3.periods, kb[0], k0[0], g3.eps_b)) <= 1e-12
     assert plan.info()["device_bytes"] - bytes0 <= 16 * (16 ** 3 + 3 * 16) + 3 * 4 * 16 + 64   # only the voxel staging was added
+    # voxel grids of changing size (non-powers of two: the defining-sum path): the staging block is replaced, not
+    # accumulated, so the plan's footprint depends on the current grid only
+    sizes = []
+    for nv in (20, 24, 20, 24, 20):
+        g = (1.0 + 5.0 * rng.random((nv, nv, nv))).astype(np.complex128)
+        plan.set_cell(g3.periods, eps_bg=1.0, eps_b=1.0, voxels=g)
+        sizes.append(plan.info()["device_bytes"])
+        c_ref = orc.coeffs_voxel(g, g3.orders, 1.0)
+        assert np.max(np.abs(plan.coeffs() - c_ref)) <= 1e-13 * np.max(np.abs(c_ref))
+    assert sizes[0] == sizes[2] == sizes[4] and sizes[1] == sizes[3] and sizes[1] > sizes[0]
     assert gsm._lib.gsm_plan_set_cell(plan._h, None) == gsm.E_INVALID
     plan.close()
 
