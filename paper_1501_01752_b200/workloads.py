@@ -142,6 +142,31 @@ def cavity_lattice(orders, kind, n_host, period=0.3) -> Geometry:
     return _geo(f"{kind}-cavity", (L, L, L), orders, [shape], e, e)
 
 
+def tetragonal_cavities(ratio, orders=(7, 7, 7), radius=0.02, fill=4.0 / 3.0 * math.pi / 27.0, n_host=1.5) -> Geometry:
+    """PAPER.md:127, :143 (Fig. 4): spherical air cavities of radius `radius` (in wavelengths) in a host of index 1.5 on a
+    simple tetragonal lattice, Lambda_x = ratio * Lambda_y,z, at the constant filling factor f = (4/3) pi / 27 = 0.155
+    (R = Lambda / 3 at equal periods): Lambda_y,z = (4 pi R^3 / (3 f ratio))^(1/3).  ratio = 1 is the isotropic crystal."""
+    lt = (4.0 / 3.0 * math.pi * radius ** 3 / (fill * ratio)) ** (1.0 / 3.0)
+    e = n_host * n_host
+    return _geo(f"tetragonal-{ratio:g}", (ratio * lt, lt, lt), orders,
+                [dict(kind=SPHERE, center=(0, 0, 0), size=(radius, 0, 0), eps=1.0)], e, e)
+
+
+def normal_surface_lines(count, seed=SEED):
+    """Cross-section of the Fresnel normal surface by the xz plane: `count` seeded propagation
+    directions s = (sin t, 0, cos t), each with the two transverse unit amplitudes - y (normal to the plane: the ordinary
+    sheet of a crystal whose axis is x) and y x s (in the plane: the extraordinary sheet).  Returns (dirs [2 count, 3],
+    pols [2 count, 3]), the two sheets of direction i at rows 2 i and 2 i + 1."""
+    rng = np.random.default_rng(seed + 5)
+    t = np.sort(rng.uniform(0.1, 0.5 * math.pi - 0.1, count))
+    dirs, pols = [], []
+    for ti in t:
+        s = np.array([math.sin(ti), 0.0, math.cos(ti)])
+        dirs += [s, s]
+        pols += [np.array([0.0, 1.0, 0.0]), np.cross([0.0, 1.0, 0.0], s)]
+    return np.array(dirs), np.array(pols)
+
+
 # ---- scan lists -----------------------------------------------------------------------------------
 DIRECTIONS = {
     # tensor entry <- (propagation axis, polarisation axis): reading R14 (cyclic)

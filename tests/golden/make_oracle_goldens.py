@@ -3,7 +3,9 @@
 configs 1, 3 and 4 (n_eff = eta / k0, eps_eff = n_eff^2: PAPER.md:54, :64; pole search Eq. 6-10, PAPER.md:64-95;
 tensor entry <-> (direction, polarisation) by DESIGN.md reading R14; two-stage mesh by reading R16).
 
-    python tests/golden/make_oracle_goldens.py [--only cfg1,cfg3,cfg4,dirs] [--threads T]
+    python tests/golden/make_oracle_goldens.py [--only cfg1,cfg3,cfg4,dirs,tetra,cfg5b] [--threads T]
+
+(cfg5b - BASELINE config 5b, one 63^3 solve - writes tests/golden/oracle_cfg5b_63.txt and is not in the default set.)
 
 Calls only oracle/ and the seeded input generators (paper_1501_01752_b200/workloads.py, which holds none of the
 method's arithmetic).  Nothing here touches the CUDA path.  Existing keys of other groups are kept, so one group can
@@ -140,6 +142,79 @@ def main():
             put(vals, f"cfg4_31_{key}", n, eps, zeta)
             write_all(vals)
             print(f"cfg4 {key} done {time.time() - t0:.0f} s: n = {n}, iters {min(its)}..{max(its)}", flush=True)
+
+    if "tetra" in groups:     # PAPER.md:127, :143 (Fig. 4): tetragonal lattice of air cavities, 7^3 orders, dense LU
+        def line(geo, c, d, pol):
+            pol = np.asarray(pol, dtype=complex)
+
+            def xi(kappa):       # reading R28: projection of the 0-th order field on the amplitude
+                return np.array([np.vdot(pol, orc.zero_order(orc.solve_dense(c, geo.periods, geo.orders, kv * d, TWO_PI,
+                                                                                geo.eps_b, pol))) for kv in kappa])
+            return orc.retrieve_two_stage(xi, TWO_PI, TETRA_WINDOW[0], TETRA_WINDOW[1])
+        dirs, pols = wl.normal_surface_lines(4)
+        for ratio in (0.7, 1.3):     # both sheets of the normal surface in the xz plane
+            geo = wl.tetragonal_cavities(ratio)
+            c = orc.coeffs_analytic(geo.periods, geo.orders, geo.shapes, geo.eps_bg, geo.eps_b)
+            for i in range(len(dirs)):
+                n, eps, zeta = line(geo, c, dirs[i], pols[i])
+                put(vals, f"tetra_{ratio:g}_surf_{i}", n, eps, zeta)
+                print(f"tetra {ratio:g} line {i} done {time.time() - t0:.0f} s: n = {n}", flush=True)
+            write_all(vals)
+        for ratio in (0.7, 0.85, 1.0, 1.15, 1.3):   # period sweep at constant filling (Fig. 4a): k || z, a = x and a = y
+            geo = wl.tetragonal_cavities(ratio)
+            c = orc.coeffs_analytic(geo.periods, geo.orders, geo.shapes, geo.eps_bg, geo.eps_b)
+            for nm, pol in (("ax", [1.0, 0, 0]), ("ay", [0, 1.0, 0])):
+                n, eps, zeta = line(geo, c, np.array([0.0, 0.0, 1.0]), pol)
+                put(vals, f"tetra_{ratio:g}_kz_{nm}", n, eps, zeta)
+                print(f"tetra sweep {ratio:g} {nm} done {time.time() - t0:.0f} s: n = {n}", flush=True)
+            write_all(vals)
+
+    if "cfg5b" in groups:     # BASELINE config 5b: one solve at 63^3 orders on the config-5 voxel composite
+        write_cfg5b(orc, wl, t0)
+
+
+TETRA_WINDOW = (1.39, 1.46)     # n_MG = 1.4213; the anisotropy splits the sheets by a few 1e-3
+
+
+CFG5B_OUT = os.path.join(HERE, "oracle_cfg5b_63.txt")
+CFG5B_SAMPLES = 4096
+
+
+def write_cfg5b(orc, wl, t0):
+    """The oracle's full GMRES (tol 1e-13, O(n^2) Toeplitz product in plain C) for ONE (k, omega) point at 63^3 orders:
+    k = (0, 0, 1.12 k0), k0 = 2 pi, a = x.  Stores the 0-th order response, ||E||_2, the iteration count and a seeded
+    sample of the field's entries (flat index into E[3][63][63][63], re, im).  About 60 applies of 1.9e11 complex
+    multiply-adds each: 20-40 minutes on 8-16 cores."""
+    geo = wl.voxel_composite((63, 63, 63), nv=128)
+    c = orc.coeffs_voxel(geo.voxels, geo.orders, geo.eps_b)
+    kb, k0, pol = np.array([0.0, 0.0, 1.12 * TWO_PI]), TWO_PI, np.array([1.0, 0.0, 0.0], dtype=complex)
+    napply = [0]
+
+    def mv(cc, x):
+        napply[0] += 1
+        print(f"cfg5b apply {napply[0]} at {time.time() - t0:.0f} s", flush=True)
+        return orc.toeplitz_matvec_c(cc, x)
+
+    E, hist, iters = orc.solve_gmres(c, geo.periods, geo.orders, kb, k0, geo.eps_b, pol, tol=1e-13, max_iters=150, matvec=mv)
+    r = orc.incident(geo.orders, pol) - orc.apply_operator(c, E, geo.periods, kb, k0, geo.eps_b, orc.toeplitz_matvec_c)
+    true_res = float(np.linalg.norm(r) / np.linalg.norm(orc.incident(geo.orders, pol)))
+    xi = orc.zero_order(E)
+    flat = E.ravel()
+    idx = np.sort(np.random.default_rng(wl.SEED + 63).choice(flat.size, CFG5B_SAMPLES, replace=False))
+    with open(CFG5B_OUT, "w") as f:
+        f.write("# BASELINE config 5b: oracle GMRES solution at 63^3 orders (voxel composite of config 5, nv = 128),\n"
+                "# k = (0, 0, 1.12 k0), k0 = 2 pi, a = x, tol 1e-13.  Written by tests/golden/make_oracle_goldens.py --only cfg5b\n"
+                "# from oracle/ alone; never edited by hand, never produced by the CUDA path.\n"
+                "# header lines: key value; then `sample <flat index into E[3][63][63][63]> <re> <im>`\n")
+        f.write(f"iters {iters}\n")
+        f.write(f"estimated_rel_resid {hist[-1]!r}\n")
+        f.write(f"true_rel_resid {true_res!r}\n")
+        f.write(f"norm_E {float(np.linalg.norm(flat))!r}\n")
+        for a in range(3):
+            f.write(f"xi{a}_re {float(xi[a].real)!r}\nxi{a}_im {float(xi[a].imag)!r}\n")
+        for i in idx:
+            f.write(f"sample {int(i)} {float(flat[i].real)!r} {float(flat[i].imag)!r}\n")
+    print(f"cfg5b done {time.time() - t0:.0f} s: {iters} iterations, true residual {true_res:.2e}, xi = {xi}", flush=True)
 
 
 if __name__ == "__main__":

@@ -17,7 +17,7 @@ torch = pytest.importorskip("torch")
 if not torch.cuda.is_available():
     pytest.skip("needs a CUDA device", allow_module_level=True)
 
-from conftest import load_oracle_golden  # noqa: E402
+from conftest import load_golden, load_oracle_golden  # noqa: E402
 from oracle import gsm_oracle as orc  # noqa: E402
 from paper_1501_01752_b200 import gsm, workloads as wl  # noqa: E402
 
@@ -544,3 +544,50 @@ def test_group_concurrent_iteration_is_bit_identical():
     assert st1 == st2 == gsm.NOT_CONVERGED and np.array_equal(i1, i2) and np.array_equal(r1, r2) and np.array_equal(s1, s2)
     assert np.all(np.delete(i1, 9) == 6)
     short.close()
+
+
+def test_tetragonal_lattice_normal_surface_and_period_sweep_vs_oracle_goldens():
+    """SURVEY 8(f) #4, the rest of the row (Fig. 4): spherical air cavities (R = 0.02 lambda) in n = 1.5 on
+    a simple tetragonal lattice at the constant filling factor 0.155.  (1) Lambda_x / Lambda_y,z = 0.7 and 1.3: BOTH sheets
+    of the Fresnel normal surface along 4 seeded directions of the xz plane - amplitude y (ordinary) and y x s
+    (extraordinary), response = projection on the amplitude (reading R28) - 8 lines per call of gsm_retrieve_neff_many,
+    against the oracle's dense-LU retrieval (tests/golden/oracle_neff.txt, group `tetra`).  (2) Five ratios at constant
+    filling through gsm_plan_set_cell, k || z with a = x and a = y, against the same goldens and the Maxwell-Garnett line."""
+    gold = load_oracle_golden()
+    mg = load_golden()["n_mg_uniaxial"]
+    dirs, pols = wl.normal_surface_lines(4)
+    plan = gsm.plan_from_geometry(wl.tetragonal_cavities(0.7), max_iters=100, max_batch=8 * 29)
+    for ratio in (0.7, 1.3):
+        geo = wl.tetragonal_cavities(ratio)
+        plan.set_cell(geo.periods, shapes=geo.shapes, eps_bg=geo.eps_bg, eps_b=geo.eps_b)
+        n, eps, zeta, ls, st = plan.retrieve_neff_many(dirs, pols.astype(complex), -1, TWO_PI, 1.39, 1.46, tol=1e-12)
+        assert st == gsm.OK and np.all(ls == gsm.OK)
+        for i in range(8):
+            key = f"tetra_{ratio:g}_surf_{i}"
+            assert abs(n[i].real - gold[key + "_neff_re"]) <= 1e-8 and abs(n[i].imag) <= 1e-9, key
+            assert abs(eps[i].real - gold[key + "_eps_re"]) <= 1e-8
+            zo = complex(gold[key + "_zeta_re"], gold[key + "_zeta_im"])
+            assert abs(zeta[i] - zo) <= 1e-6 * abs(zo)
+        # uniaxial crystal, axis x: the ordinary sheet is (nearly) a circle, the extraordinary one is not, and the two
+        # approach each other as s turns towards the axis (rows are sorted by the angle between s and z)
+        no, ne = n[0::2].real, n[1::2].real
+        assert np.ptp(no) <= 5e-5 and np.ptp(ne) >= 1e-3
+        assert np.all(np.diff(np.abs(ne - no)) < 0)
+        assert (ne[0] > no[0]) == (ratio < 1.0)
+    zdir = np.array([[0.0, 0.0, 1.0], [0.0, 0.0, 1.0]])
+    xy = np.array([[1.0, 0, 0], [0, 1.0, 0]], dtype=complex)
+    nx, ny = [], []
+    for ratio in (0.7, 0.85, 1.0, 1.15, 1.3):
+        geo = wl.tetragonal_cavities(ratio)
+        plan.set_cell(geo.periods, shapes=geo.shapes, eps_bg=geo.eps_bg, eps_b=geo.eps_b)
+        n, eps, zeta, ls, st = plan.retrieve_neff_many(zdir, xy, -1, TWO_PI, 1.39, 1.46, tol=1e-12)
+        assert st == gsm.OK and np.all(ls == gsm.OK)
+        for i, nm in enumerate(("ax", "ay")):
+            assert abs(n[i].real - gold[f"tetra_{ratio:g}_kz_{nm}_neff_re"]) <= 1e-8
+        nx.append(n[0].real); ny.append(n[1].real)
+    nx, ny = np.array(nx), np.array(ny)
+    assert abs(nx[2] - ny[2]) <= 1e-10                         # equal periods: isotropic
+    assert 0.0 < nx[2] - mg < 3e-3                             # PAPER.md:127: finite periods raise the index above Maxwell-Garnett
+    assert np.all(np.diff(nx) < 0) and np.all(np.diff(ny) > 0)  # extraordinary falls, ordinary rises with Lambda_x / Lambda_y,z
+    assert nx[-1] < mg                                         # "one of the effective indices ... can become lower than" the MG value
+    plan.close()
