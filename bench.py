@@ -430,6 +430,40 @@ def run_gsm(args):
     fft_grid = list(plan_h.info()["fft_grid"])
     plan_h.close()
 
+    def solve_report(p, kbs_, k0s_, pols_, tol, reps, grid_pts):
+        """`reps` timed scans of the points given (one lock-step batch, zero start) with profiling off, then one more with a
+        CUDA event pair around every launch: time, kernel split, dominant kernel and whole path against the HBM roof
+        (SURVEY 8(d) B_solve = (m(m+1)/2 + 3m + 1) V + m |Chat| per solve)."""
+        peak_, _ = _peaks()
+        nb = len(k0s_)
+        p.scan(kbs_, k0s_, pols_, tol=tol)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record(stream)
+        for _ in range(reps):
+            _, its_, res_, _ = p.scan(kbs_, k0s_, pols_, tol=tol)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        ms_ = r0.elapsed_time(r1) / reps
+        p.profile(True); p.profile_read(reset=True)
+        p.scan(kbs_, k0s_, pols_, tol=tol)
+        torch.cuda.synchronize()
+        pr_ = {k: v for k, v in p.profile_read(reset=True).items() if v[0] > 0 and k != "plan"}
+        p.profile(False)
+        Vn = 16.0 * 3 * p.n
+        b_ = float(np.sum((its_ * (its_ + 1.0) / 2 + 3.0 * its_ + 1.0) * Vn)) + float(np.mean(its_)) * 16.0 * grid_pts
+        dom_ = max(pr_, key=lambda k: pr_[k][1])
+        kms_ = sum(v[1] for v in pr_.values())
+        return {"batch": nb, "ms": ms_, "solves_per_s": nb * 1e3 / ms_, "iters": [int(i) for i in its_],
+                "max_true_resid": float(np.max(res_)),
+                "path_roofline": {"algorithmic_GBps": b_ / (ms_ * 1e-3) / 1e9, "frac": b_ / (ms_ * 1e-3) / 1e9 / peak_},
+                "roofline": {"bound": "hbm", "kernel": dom_, "achieved": pr_[dom_][2] / (pr_[dom_][1] * 1e-3) / 1e9, "peak": peak_,
+                             "unit": "GB/s", "frac": pr_[dom_][2] / (pr_[dom_][1] * 1e-3) / 1e9 / peak_, "launches": pr_[dom_][0],
+                             "avg_launch_ms": pr_[dom_][1] / pr_[dom_][0], "share_of_step": pr_[dom_][1] / kms_, "traffic": None},
+                "profiled_pass_ms": kms_, "launches": int(sum(v[0] for v in pr_.values())),
+                "kernel_ms": {k: v[1] for k, v in pr_.items()},
+                "kernel_GBps": {k: (v[2] / (v[1] * 1e-3) / 1e9 if v[1] > 0 and v[2] > 0 else None) for k, v in pr_.items()}}
+
     # ---- config 5b: single solves at 63^3 orders (FFT grid 128^3), informational, rank 0 only ------------------------
     c5b = None
     if rank == 0:
@@ -461,8 +495,14 @@ def run_gsm(args):
                "apply_ms": ap_ms, "applies_per_s": 1e3 / ap_ms,
                "apply_algorithmic_GBps": (2 * V63 + 16.0 * 128 ** 3) / (ap_ms * 1e-3) / 1e9,
                "note": "working set of one apply (x, y, W, Chat ~ 150 MB) is about the size of L2"}
+        c5b["single_solve"] = solve_report(p63, kb63[None], np.array([TWO_PI]), pol63[None], TOL, 3, 128 ** 3)
         p63.close()
         del x63, y63
+        torch.cuda.empty_cache()
+        p63b = gsm.plan_from_geometry(geo63, max_iters=MAX_ITERS, max_batch=8, stream=stream)
+        kb8, k08, pol8 = wl.scan_points(wl.kappa_mesh(N_LO, N_HI, 8), 2, 0)
+        c5b["batch_of_8"] = solve_report(p63b, kb8, k08, pol8, TOL, 2, 128 ** 3)
+        p63b.close()
         torch.cuda.empty_cache()
         # ---- the two large sizes of the paper's Table 1 as single solves (context: PAPER.md:111-115 gives 2.2 s and 114 s
         # on a GTX Titan, the latter with the GMRES basis streamed from host RAM); informational
@@ -477,7 +517,8 @@ def run_gsm(args):
             s1.record(stream)
             torch.cuda.synchronize()
             large.append({"orders": [N, N, N], "unknowns": 3 * N ** 3, "solve_ms": s0.elapsed_time(s1), "iters": int(itl),
-                          "true_resid": float(resl), "device_GB": pl_.info()["device_bytes"] / 1e9})
+                          "true_resid": float(resl), "device_GB": pl_.info()["device_bytes"] / 1e9,
+                          "report": solve_report(pl_, kbl[None], np.array([TWO_PI]), poll[None], 1e-8, 1, (2 * N) ** 3)})
             pl_.close()
             torch.cuda.empty_cache()
         c5b["large_orders_single_solve"] = large

@@ -32,8 +32,6 @@ def build_cuda(force=False, verbose=False):
     cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-o", LIB] + srcs
-    extra = os.environ.get("GSM_NVCC_FLAGS", "").split()   # tuning experiments only (e.g. -DXY64_MINB=2)
-    cmd[1:1] = extra
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)

@@ -26,9 +26,7 @@ namespace gsm {
 //   y inverse : mirror of y forward, stores straight to W
 // chat64 is Chat permuted so that the 8 lanes of a group read 8 consecutive coefficients:
 //   chat64[((pos3 * 64 + r) * 8 + q) * 8 + u] = Chat[pos3][pos1 = 8u + q][pos2 = r].
-#ifndef XY64_MINB
 #define XY64_MINB 2   // measured: 2 CTAs/SM at 122 registers (no spills) beats 3 CTAs/SM at 80 (46 vs 52 ms)
-#endif
 __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, cplx* __restrict__ W,
                                                            const cplx* __restrict__ chat64,
                                                            const int* __restrict__ active) {
@@ -113,9 +111,7 @@ __global__ void __launch_bounds__(256, XY64_MINB) xy_conv64_kernel(ApplyGeom g, 
 // CTA = 32 consecutive z-lines of one (b, c).  Each group loads its line's <= 32 inputs straight from x (contiguous),
 // transforms, and drops the 64 outputs into a [pos3][32 lines] tile (columns rotated by pos3/8: conflict-free), which
 // is then written to W[b][c][pos3][l] as 512-byte rows.
-#ifndef ZF64_MINB
 #define ZF64_MINB 4
-#endif
 template <bool HFORM>
 __global__ void __launch_bounds__(256, ZF64_MINB) z_forward64_kernel(ApplyGeom g, const cplx* __restrict__ x,
                                                                      cplx* __restrict__ W, const double* __restrict__ kvec,

@@ -283,9 +283,6 @@ cudaError_t arnoldi_cluster_plan(const KrylovDims& d, int* cs_out, int* chunk_ou
     if (e != cudaSuccess || nclusters < 1) { cudaGetLastError(); return cudaSuccess; }
     *cs_out = cs;
     *chunk_out = chunk;
-#ifdef MGS_NCL_CAP   // tuning experiments only
-    if (nclusters > MGS_NCL_CAP) nclusters = MGS_NCL_CAP;
-#endif
     *nclusters_out = nclusters;
     return cudaSuccess;
 }

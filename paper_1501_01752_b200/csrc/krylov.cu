@@ -99,10 +99,36 @@ __global__ void __launch_bounds__(KT) sweep_dots_kernel(KrylovDims d, KrylovStat
     }
 }
 
-// per solve: reduce the partials, store the Gram row, run the MGS recurrence -> hcol[0..j]
-// HS_T threads: warp w reduces the partials of entries i = w, w + HS_T/32, ... (lanes stride over the chunks, fixed
-// shuffle tree: deterministic), then warp 0 runs the recurrence.
+// Reduction of sweep 1's partials over the chunks, one CTA per (entry i, solve b): hcol[b][i] = <v_i, w> (before the
+// recurrence) and gram[i][j] = <v_i, v_j>.  Threads stride over the chunks, then a fixed shuffle / shared-memory tree:
+// deterministic.  (One CTA per solve doing all j + 1 entries took 48 us per iteration at 63^3 orders and 1.4 ms at 256^3,
+// profiles/ncu_full_r3_63.txt: a chain of dependent load round trips on one SM.)
 #define HS_T 256
+__global__ void __launch_bounds__(HS_T) hreduce_kernel(KrylovDims d, KrylovState s, int j) {
+    const int i = blockIdx.x, b = blockIdx.y;
+    if (!s.active[b]) return;
+    __shared__ double red[HS_T / 32][4];
+    const cplx* p = s.part + ((long)b * 2 * d.ld + 2 * i) * d.nchunk;
+    double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
+    for (int c = threadIdx.x; c < d.nchunk; c += HS_T) {
+        const cplx a = p[c], g = p[d.nchunk + c];
+        a0 += a.x; a1 += a.y; g0 += g.x; g1 += g.y;
+    }
+    a0 = warp_sum(a0); a1 = warp_sum(a1); g0 = warp_sum(g0); g1 = warp_sum(g1);
+    if ((threadIdx.x & 31) == 0) {
+        double* r = red[threadIdx.x >> 5];
+        r[0] = a0; r[1] = a1; r[2] = g0; r[3] = g1;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a0 = a1 = g0 = g1 = 0;
+        for (int q = 0; q < HS_T / 32; ++q) { a0 += red[q][0]; a1 += red[q][1]; g0 += red[q][2]; g1 += red[q][3]; }
+        s.hcol[(long)b * d.ld + i] = make_double2(a0, a1);
+        s.gram[(long)b * d.ld * d.ld + (long)i * d.ld + j] = make_double2(g0, g1);
+    }
+}
+
+// per solve: run the MGS recurrence on the reduced inner products -> hcol[0..j] (warp 0; the others help staging)
 __global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState s, int batch, int j, int stage) {
     const int b = blockIdx.x;
     if (!s.active[b]) return;
@@ -110,19 +136,7 @@ __global__ void __launch_bounds__(HS_T) hsolve_kernel(KrylovDims d, KrylovState 
     cplx* dd = reinterpret_cast<cplx*>(smem_raw);   // [ld]
     cplx* gT = s.gram + (long)b * d.ld * d.ld;      // gT[k*ld + i] = <v_k, v_i>, k <= i
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int i = warp; i <= j; i += HS_T / 32) {
-        double a0 = 0, a1 = 0, g0 = 0, g1 = 0;
-        const cplx* p = s.part + ((long)b * 2 * d.ld + 2 * i) * d.nchunk;
-        for (int c = lane; c < d.nchunk; c += 32) {
-            const cplx a = p[c], g = p[d.nchunk + c];
-            a0 += a.x; a1 += a.y; g0 += g.x; g1 += g.y;
-        }
-        a0 = warp_sum(a0); a1 = warp_sum(a1); g0 = warp_sum(g0); g1 = warp_sum(g1);
-        if (lane == 0) {
-            dd[i] = make_double2(a0, a1);
-            gT[(long)i * d.ld + j] = make_double2(g0, g1);
-        }
-    }
+    for (int i = threadIdx.x; i <= j; i += HS_T) dd[i] = s.hcol[(long)b * d.ld + i];
     // stage the Gram rows the recurrence needs (k < i <= j) in shared memory: the recurrence is a chain of j dependent
     // steps, and a global-memory load per step would cost an L2 round trip each
     const cplx* gs = gT;                             // stage == 0: basis too long for shared memory, read the rows from global
@@ -539,6 +553,10 @@ cudaError_t launch_sweep_dots(const KrylovDims& d, const KrylovState& s, int bat
     return cudaGetLastError();
 }
 cudaError_t launch_hsolve(const KrylovDims& d, const KrylovState& s, int batch, int j, cudaStream_t st, Profiler* prof) {
+    { ProfScope pr_(prof, KC_HSOLVE, st);
+      hreduce_kernel<<<dim3(j + 1, batch), HS_T, 0, st>>>(d, s, j);
+      const cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) return e; }
     ProfScope ps_(prof, KC_HSOLVE, st);
     size_t smem = sizeof(cplx) * d.ld * (size_t)(j + 1);
     const int stage = smem <= 200 * 1024;
