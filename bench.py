@@ -551,6 +551,10 @@ def run_gsm(args):
     cpu_t, cpu_it, cores = oracle_solve_once(geo, kb[0], k0[0], pol[0])
     cpu_apply_t = oracle_apply_once(geo, kb[0], k0[0])
     cpu_small = oracle_small_sizes()
+    # SURVEY 8(d) / BASELINE.md 2: one oracle apply at 63^3 orders measured (1.9e11 complex multiply-adds); the 63^3 solve and
+    # the 256-solve batch at 31^3 are extrapolated from measured pieces and labelled as such
+    cpu_apply63_t = oracle_apply_once(wl.voxel_composite((63, 63, 63), nv=128), np.array([0.0, 0.0, 1.12 * TWO_PI]), TWO_PI, reps=1)
+    it63_gpu = c5b["single_solve"]["iters"][0] if c5b else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -615,7 +619,13 @@ def run_gsm(args):
                          "gpu_over_oracle_like_for_like": value / world * cpu_t,
                          "ratio_note": "value per GPU / this oracle figure: both are full GMRES solves from x0 = 0 of points of "
                                        "the same list (a GPU-over-slow-CPU figure, not a kernel-quality one)",
-                         "other_sizes": cpu_small},
+                         "other_sizes": cpu_small,
+                         "apply_63cubed_s": cpu_apply63_t,
+                         "apply_63cubed_sample": "one operator apply at 63^3 orders (config 5b), measured once after one warm-up apply",
+                         "solve_63cubed_s_extrapolated": cpu_apply63_t * (it63_gpu + 1) if it63_gpu else None,
+                         "solve_63cubed_note": "EXTRAPOLATED: measured apply x (iterations of the GPU solve of the same point + 1)",
+                         "batch_256_at_31cubed_s_extrapolated": cpu_t * BATCH,
+                         "batch_256_note": "EXTRAPOLATED: the one measured 31^3 solve x 256"},
     }
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -4,6 +4,8 @@ oracle can afford it, the oracle's own full GMRES above that).
 Bars (BASELINE.json north_star): relative L2 field error <= 1e-9, true Krylov residual <= 1e-10, retrieved
 eps_eff within 1e-8.  Solves run to tol 1e-12 (reading R10: field error <= cond(A) x residual).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -357,6 +359,42 @@ def _check_equation_rows(geo, c, F, kb, k0, pol, nsamp):
             lhs = F[b][(slice(None),) + s] - (kb2 * T - km * np.dot(km, T)) / (np.dot(km, km) - kb2)
             rhs = pol[b] if s == i0 else np.zeros(3)
             assert np.max(np.abs(lhs - rhs)) <= 1e-9 * max(1.0, scale)
+
+
+def test_config5b_63cubed_single_solve_vs_oracle_solution():
+    """BASELINE config 5b at the north_star's tolerance: one solve at 63^3 orders against the ORACLE'S OWN SOLUTION of the same
+    point (full GMRES to 1e-13 with the O(n^2) Toeplitz product, ~45 minutes of host time, stored once by
+    tests/golden/make_oracle_goldens.py --only cfg5b): the 0-th order response, the norm of the field and 4096 seeded
+    entries of it.  Field entries within 1e-9 of the field's rms entry, sampled relative L2 error, xi and norm within 1e-9."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_cfg5b_63.txt")
+    head, idx, val = {}, [], []
+    with open(path) as f:
+        for line in f:
+            t = line.split("#")[0].split()
+            if not t:
+                continue
+            if t[0] == "sample":
+                idx.append(int(t[1])); val.append(complex(float(t[2]), float(t[3])))
+            else:
+                head[t[0]] = float(t[1])
+    idx, val = np.array(idx), np.array(val)
+    assert len(idx) == 4096 and head["true_rel_resid"] <= 1e-12
+    geo = wl.voxel_composite((63, 63, 63), nv=128)
+    plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=1)
+    kb = np.array([0.0, 0.0, 1.12 * TWO_PI]); pol = np.array([1.0, 0, 0], dtype=complex)
+    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    assert st == gsm.OK and resid <= 1e-10 and abs(iters - int(head["iters"])) <= 8
+    F = E.cpu().numpy()
+    n3 = F.size
+    rms = head["norm_E"] / np.sqrt(n3)
+    got = F.ravel()[idx]
+    assert np.max(np.abs(got - val)) <= 1e-9 * rms
+    assert np.linalg.norm(got - val) / np.linalg.norm(val) <= 1e-9
+    assert abs(np.linalg.norm(F) - head["norm_E"]) <= 1e-9 * head["norm_E"]
+    xi = orc.zero_order(F)
+    xo = np.array([complex(head[f"xi{a}_re"], head[f"xi{a}_im"]) for a in range(3)])
+    assert np.max(np.abs(xi - xo)) <= 1e-9 * np.max(np.abs(xo))
+    plan.close()
 
 
 def test_config5b_63cubed_single_solve_satisfies_the_equation():
