@@ -207,7 +207,7 @@ def write_cfg5b(orc, wl, t0):
                 "# from oracle/ alone; never edited by hand, never produced by the CUDA path.\n"
                 "# header lines: key value; then `sample <flat index into E[3][63][63][63]> <re> <im>`\n")
         f.write(f"iters {iters}\n")
-        f.write(f"estimated_rel_resid {hist[-1]!r}\n")
+        f.write(f"estimated_rel_resid {float(hist[-1])!r}\n")
         f.write(f"true_rel_resid {true_res!r}\n")
         f.write(f"norm_E {float(np.linalg.norm(flat))!r}\n")
         for a in range(3):

@@ -378,13 +378,13 @@ def test_config5b_63cubed_single_solve_vs_oracle_solution():
             if t[0] == "sample":
                 idx.append(int(t[1])); val.append(complex(float(t[2]), float(t[3])))
             else:
-                head[t[0]] = float(t[1])
+                head[t[0]] = float(t[1].replace("np.float64(", "").rstrip(")"))   # numpy 2 prints its scalars as np.float64(..)
     idx, val = np.array(idx), np.array(val)
-    assert len(idx) == 4096 and head["true_rel_resid"] <= 1e-12
+    assert len(idx) == 4096 and head["true_rel_resid"] <= 1e-11 and head["estimated_rel_resid"] <= 1e-13
     geo = wl.voxel_composite((63, 63, 63), nv=128)
     plan = gsm.plan_from_geometry(geo, max_iters=100, max_batch=1)
     kb = np.array([0.0, 0.0, 1.12 * TWO_PI]); pol = np.array([1.0, 0, 0], dtype=complex)
-    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-12)
+    E, hist, iters, resid, st = plan.solve(kb, TWO_PI, pol, tol=1e-13)          # the oracle's own tolerance
     assert st == gsm.OK and resid <= 1e-10 and abs(iters - int(head["iters"])) <= 8
     F = E.cpu().numpy()
     n3 = F.size
